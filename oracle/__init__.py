@@ -1,0 +1,210 @@
+"""ctypes front end of the fp64 CPU oracle (oracle/tacaw_oracle.c).  TEST INFRASTRUCTURE, NOT PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
+this package.  It never imports paper_2607_02236_b200's CUDA binding and shares no code with it.
+Every function is a marshalling shim around the C routine of the same name; the arithmetic and the
+paper citations live in the C file's header.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from typing import List, Optional, Sequence, Tuple
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "tacaw_oracle.c")
+_LIB = os.path.join(_HERE, "liboracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile liboracle.so with gcc (OpenMP over independent slices / waves / series)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + f".tmp{os.getpid()}"
+        subprocess.check_call(["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", "-std=c11", "-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = C.CDLL(_LIB)
+        _lib.oracle_bose.restype = C.c_double
+        _lib.oracle_bose.argtypes = [C.c_double]
+    return _lib
+
+
+def _p(a: np.ndarray):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def num_threads() -> int:
+    return int(lib().oracle_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    lib().oracle_set_num_threads(C.c_int(n))
+
+
+def set_fft_mode(mode: int) -> None:
+    """0 auto (naive DFT for n<=64, radix-2 above), 1 force naive DFT, 2 force radix-2."""
+    lib().oracle_set_fft_mode(C.c_int(mode))
+
+
+def dft_naive(x: np.ndarray, sign: int) -> np.ndarray:
+    x = np.ascontiguousarray(x, dtype=np.complex128)
+    out = np.empty_like(x)
+    lib().oracle_dft_naive(C.c_int(x.size), _p(x), _p(out), C.c_int(sign))
+    return out
+
+
+def fft_radix2(x: np.ndarray, sign: int) -> np.ndarray:
+    x = np.array(x, dtype=np.complex128, order="C")
+    lib().oracle_fft_radix2(C.c_int(x.size), _p(x), C.c_int(sign))
+    return x
+
+
+def fft2(a: np.ndarray, sign: int) -> np.ndarray:
+    """sign=-1 forward (unscaled), +1 inverse (1/(nx ny))."""
+    a = np.array(a, dtype=np.complex128, order="C")
+    ny, nx = a.shape
+    lib().oracle_fft2(C.c_int(ny), C.c_int(nx), _p(a), C.c_int(sign))
+    return a
+
+
+def build_slices(nx: int, ny: int, lx: float, ly: float, pos: np.ndarray, species: np.ndarray,
+                 a: np.ndarray, b: np.ndarray, dz: float, nslices: int, z0: float, sigma: float,
+                 bandlimit: int = 1, pot_mode: int = 1, want_v: bool = False, want_vq: bool = False):
+    """Returns dict(trans [S][ny][nx] c128, n_clamped, max_imag[, v][, vq])."""
+    pos = np.ascontiguousarray(pos, dtype=np.float64)
+    species = np.ascontiguousarray(species, dtype=np.int32)
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    b = np.ascontiguousarray(b, dtype=np.float64)
+    trans = np.empty((nslices, ny, nx), dtype=np.complex128)
+    v = np.empty((nslices, ny, nx), dtype=np.float64) if want_v else None
+    vq = np.empty((nslices, ny, nx), dtype=np.complex128) if want_vq else None
+    ncl = C.c_int(0)
+    mi = C.c_double(0.0)
+    rc = lib().oracle_build_slices(
+        C.c_int(nx), C.c_int(ny), C.c_double(lx), C.c_double(ly), _p(pos), _p(species),
+        C.c_int(pos.shape[0]), C.c_int(a.shape[0]), _p(a), _p(b), C.c_double(dz), C.c_int(nslices),
+        C.c_double(z0), C.c_double(sigma), C.c_int(bandlimit), C.c_int(pot_mode), _p(trans),
+        _p(v) if want_v else None, _p(vq) if want_vq else None, C.byref(ncl), C.byref(mi))
+    if rc != 0:
+        raise RuntimeError(f"oracle_build_slices failed: {rc}")
+    out = dict(trans=trans, n_clamped=int(ncl.value), max_imag=float(mi.value))
+    if want_v:
+        out["v"] = v
+    if want_vq:
+        out["vq"] = vq
+    return out
+
+
+def make_probes(nx: int, ny: int, lx: float, ly: float, lam: float, probe_xy: np.ndarray,
+                alpha_rad: float) -> np.ndarray:
+    probe_xy = np.ascontiguousarray(probe_xy, dtype=np.float64).reshape(-1, 2)
+    waves = np.empty((probe_xy.shape[0], ny, nx), dtype=np.complex128)
+    rc = lib().oracle_make_probes(C.c_int(nx), C.c_int(ny), C.c_double(lx), C.c_double(ly), C.c_double(lam),
+                                  _p(probe_xy), C.c_int(probe_xy.shape[0]), C.c_double(alpha_rad), _p(waves))
+    if rc != 0:
+        raise RuntimeError(f"oracle_make_probes failed: {rc}")
+    return waves
+
+
+def propagate(lx: float, ly: float, lam: float, bandlimit: int, waves: np.ndarray,
+              wave_frame: Optional[Sequence[int]], trans: Sequence[Sequence[np.ndarray]], dz: float,
+              output_space: int = 0, want_norms: bool = False):
+    """waves [nw][ny][nx] c128 (copied).  trans[f][k] = c128 [S_k][ny][nx] for in-flight frame f and
+    z-segment k.  Returns the propagated waves (and norms [nw][S+1] if asked)."""
+    waves = np.array(waves, dtype=np.complex128, order="C")
+    nw, ny, nx = waves.shape
+    nframes = len(trans)
+    nseg = len(trans[0])
+    keep = [[np.ascontiguousarray(t, dtype=np.complex128) for t in fr] for fr in trans]
+    nsl = np.array([t.shape[0] for t in keep[0]], dtype=np.int32)
+    ptrs = (C.c_void_p * (nframes * nseg))()
+    for f in range(nframes):
+        assert len(keep[f]) == nseg
+        for k in range(nseg):
+            assert keep[f][k].shape == (nsl[k], ny, nx)
+            ptrs[f * nseg + k] = keep[f][k].ctypes.data
+    wf = np.ascontiguousarray(wave_frame if wave_frame is not None else np.zeros(nw), dtype=np.int32)
+    total = int(nsl.sum())
+    norms = np.empty((nw, total + 1), dtype=np.float64) if want_norms else None
+    rc = lib().oracle_propagate(C.c_int(nx), C.c_int(ny), C.c_double(lx), C.c_double(ly), C.c_double(lam),
+                                C.c_int(bandlimit), _p(waves), _p(wf), C.c_int(nw), ptrs, C.c_int(nframes),
+                                _p(nsl), C.c_int(nseg), C.c_double(dz), C.c_int(output_space),
+                                _p(norms) if want_norms else None)
+    if rc != 0:
+        raise RuntimeError(f"oracle_propagate failed: {rc}")
+    return (waves, norms) if want_norms else waves
+
+
+ROI_MODES = {"full": 0, "disc": 1, "annulus": 2, "rect": 3}
+
+
+def make_roi(nx: int, ny: int, lx: float, ly: float, lam: float, mode: str, params_rad: Sequence[float]) -> np.ndarray:
+    params = np.ascontiguousarray(list(params_rad) + [0.0] * 4, dtype=np.float64)
+    cnt = C.c_int64(0)
+    args = [C.c_int(nx), C.c_int(ny), C.c_double(lx), C.c_double(ly), C.c_double(lam), C.c_int(ROI_MODES[mode]), _p(params)]
+    rc = lib().oracle_make_roi(*args, None, C.byref(cnt))
+    if rc != 0:
+        raise RuntimeError(f"oracle_make_roi failed: {rc}")
+    idx = np.empty(cnt.value, dtype=np.int32)
+    lib().oracle_make_roi(*args, _p(idx), C.byref(cnt))
+    return idx
+
+
+def accumulate(qwaves: np.ndarray, wave_probe: Sequence[int], wave_frame: Sequence[int], roi_idx: np.ndarray,
+               buf: np.ndarray) -> None:
+    """buf [nprobes][nframes][nroi] c128, updated in place."""
+    qwaves = np.ascontiguousarray(qwaves, dtype=np.complex128)
+    nw, ny, nx = qwaves.shape
+    wp = np.ascontiguousarray(wave_probe, dtype=np.int32)
+    wf = np.ascontiguousarray(wave_frame, dtype=np.int32)
+    roi_idx = np.ascontiguousarray(roi_idx, dtype=np.int32)
+    assert buf.dtype == np.complex128 and buf.flags.c_contiguous and buf.shape[2] == roi_idx.size
+    rc = lib().oracle_accumulate(C.c_int(nx), C.c_int(ny), _p(qwaves), C.c_int(nw), _p(wp), _p(wf), _p(roi_idx),
+                                 C.c_int64(roi_idx.size), _p(buf), C.c_int(buf.shape[0]), C.c_int(buf.shape[1]))
+    if rc != 0:
+        raise RuntimeError(f"oracle_accumulate failed: {rc}")
+
+
+def bose(x: float) -> float:
+    return float(lib().oracle_bose(C.c_double(x)))
+
+
+def window(kind: int, nframes: int) -> np.ndarray:
+    w = np.empty(nframes, dtype=np.float64)
+    lib().oracle_window(C.c_int(kind), C.c_int(nframes), _p(w))
+    return w
+
+
+def energy_axis(nframes: int, dt_fs: float, emin: float = -np.inf, emax: float = np.inf) -> Tuple[np.ndarray, np.ndarray]:
+    E = np.empty(nframes, dtype=np.float64)
+    bins = np.empty(nframes, dtype=np.int32)
+    lib().oracle_energy_axis.restype = C.c_int
+    n = lib().oracle_energy_axis(C.c_int(nframes), C.c_double(dt_fs), C.c_double(emin), C.c_double(emax), _p(E), _p(bins))
+    return E[:n].copy(), bins[:n].copy()
+
+
+def spectrum(buf: np.ndarray, dt_fs: float, window_kind: int, temperature_K: float,
+             emin: float = -np.inf, emax: float = np.inf) -> Tuple[np.ndarray, np.ndarray]:
+    """buf [P][T][Q] c128 -> (I [P][nE][Q] f64, E [nE] meV ascending)."""
+    buf = np.ascontiguousarray(buf, dtype=np.complex128)
+    P, T, Q = buf.shape
+    E, _ = energy_axis(T, dt_fs, emin, emax)
+    I = np.empty((P, E.size, Q), dtype=np.float64)
+    Eo = np.empty(E.size, dtype=np.float64)
+    nE = C.c_int(0)
+    rc = lib().oracle_spectrum(_p(buf), C.c_int(P), C.c_int64(Q), C.c_int(T), C.c_double(dt_fs), C.c_int(window_kind),
+                               C.c_double(temperature_K), C.c_double(emin), C.c_double(emax), _p(I), _p(Eo), C.byref(nE))
+    if rc != 0:
+        raise RuntimeError(f"oracle_spectrum failed: {rc}")
+    assert nE.value == E.size
+    return I, Eo
