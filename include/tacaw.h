@@ -1,0 +1,154 @@
+/* tacaw.h -- C ABI of the B200-native TACAW hot path (libtacaw.so, hand-written sm_100a CUDA).
+ *
+ * Method: arxiv/paper_2607_02236 ("torched-TACAW").  Citations are PAPER.md line numbers.
+ *   I(q,E) ~ beta E/(1-exp(-beta E)) |phi_MD(q,E)|^2                      Eq.(1), :35-40
+ *   one batch = multislice on each snapshot, gather of the exit wave inside a q-ROI, window,
+ *   time->energy FFT, |.|^2, quantum-statistics factor                      :122, :132, :142
+ * The multislice formulas (the paper delegates them to pyms, :94) are the textbook scheme that
+ * DESIGN.md section 3 spells out (steps O1-O10, readings G1-G21).
+ *
+ * Conventions
+ *   - Arrays are row-major [iy][ix], x fastest.  complex64 = interleaved (re, im) float.
+ *   - Frequency index h = ix for ix < nx/2, else ix - nx (same for k, iy).  q = (h/lx, k/ly) in
+ *     1/Angstrom (no 2 pi).  Forward transform uses exp(-2 pi i ...); inverse carries 1/(nx ny).
+ *   - nx, ny: powers of two in [16, 2048] (they may differ).
+ *   - Every "d_" pointer is DEVICE memory owned by the caller; the library never frees or
+ *     reallocates it.  The library owns only the context (tables and a small scratch buffer).
+ *   - `stream` is a cudaStream_t cast to void* (NULL = default stream).  Calls enqueue work on it
+ *     and return without synchronising unless stated; host outputs are written before return.
+ *   - Every call returns TACAW_OK (0) or a negative TACAW_E_* code; nothing throws or exits.
+ *     tacaw_last_error(ctx) gives a message for the last failure on that context.
+ *   - There is no CPU fallback: without a CUDA device tacaw_create fails with TACAW_E_CUDA.
+ */
+#ifndef TACAW_H
+#define TACAW_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TACAW_OK 0
+#define TACAW_E_ARG (-1)         /* bad argument (null pointer, negative size, index out of range) */
+#define TACAW_E_UNSUPPORTED (-2) /* grid or series length outside the supported set */
+#define TACAW_E_NOMEM (-3)       /* scratch allocation failed */
+#define TACAW_E_CUDA (-4)        /* CUDA runtime error (message in tacaw_last_error) */
+
+typedef struct tacaw_ctx tacaw_ctx;
+
+typedef struct {
+    int nx, ny;       /* grid points */
+    double lx_A, ly_A; /* periodic cell edge lengths, Angstrom */
+} tacaw_grid;
+
+typedef struct {
+    double lambda_A;          /* electron wavelength, Angstrom */
+    double sigma_rad_per_VA;  /* interaction constant, rad/(V Angstrom) */
+    int bandlimit;            /* 1: sharp mask at 2/3 of the smaller Nyquist (O5, reading G3); 0: none */
+} tacaw_beam;
+
+typedef struct {
+    int nspecies;
+    const double *a; /* HOST [nspecies][4], V*Angstrom^3 */
+    const double *b; /* HOST [nspecies][4], Angstrom^2   : f_s(q^2) = sum_i a_si exp(-b_si q^2) */
+} tacaw_species;
+
+/* ROI predicates for tacaw_make_roi (O8). */
+#define TACAW_ROI_FULL 0
+#define TACAW_ROI_DISC 1     /* params: theta_o                    lambda^2 q^2 <= theta_o^2       */
+#define TACAW_ROI_ANNULUS 2  /* params: theta_i, theta_o                                            */
+#define TACAW_ROI_RECT 3     /* params: txmin, txmax, tymin, tymax  (the paper's minmax_mrad), rad  */
+
+#define TACAW_WINDOW_RECT 0
+#define TACAW_WINDOW_HANN 1  /* periodic Hann, w_f = 1/2 - 1/2 cos(2 pi f/T) (:142, :182; reading G9) */
+
+/* Library version string and the SM architecture it was compiled for ("sm_100a"). */
+const char *tacaw_version(void);
+
+/* Create a context on CUDA device `device`: twiddle tables, band-limit column extents.
+ * Fails with TACAW_E_UNSUPPORTED for grids outside the supported set, TACAW_E_CUDA without a GPU. */
+int tacaw_create(tacaw_ctx **ctx, const tacaw_grid *grid, const tacaw_beam *beam, int device);
+int tacaw_destroy(tacaw_ctx *ctx);
+const char *tacaw_last_error(const tacaw_ctx *ctx);
+
+/* Number of kernels this context has launched since creation (bench.py's gpu_launches). */
+int64_t tacaw_launch_count(const tacaw_ctx *ctx);
+
+/* O1-O3 (PAPER.md:162 one atomic layer per slice; :219 planes at 1/4, 3/4; :505 "transmission
+ * functions ... evaluated for each multislice run").
+ *   n_j = clamp(floor((z_j - z0)/dz), 0, S-1)                                   (atoms outside are
+ *         clamped to the first/last slice and counted -- never wrapped, :219)
+ *   V_n[h,k] = sum_{j in n} f_s(q^2) exp(-2 pi i (h x_j/lx + k y_j/ly))   on in-band (h,k)
+ *   v_n = Re{ IFFT2(V_n) nx ny/(lx ly) },   t_n = exp(i sigma v_n)
+ * d_pos_A   DEVICE double [natoms][3] (Angstrom);  d_species DEVICE int32 [natoms] in [0,nspecies)
+ * d_trans   DEVICE complex64 [nslices][ny][nx], written
+ * n_clamped HOST, optional; when non-NULL the call synchronises the stream before returning. */
+int tacaw_build_slices(tacaw_ctx *ctx, const double *d_pos_A, const int32_t *d_species, int natoms,
+                       const tacaw_species *species, double slice_thickness_A, int nslices, double z0_A,
+                       void *d_trans, int *n_clamped, void *stream);
+
+/* O4 probes: Psi0[h,k] = A exp(-2 pi i (h x_p/lx + k y_p/ly)), A = 1 iff
+ * lambda^2 q^2 <= alpha^2 (alpha = 0: plane wave), inverse transformed and scaled to unit norm.
+ * probe_xy_A HOST double [nprobes][2];  d_waves DEVICE complex64 [nprobes][ny][nx], written. */
+int tacaw_make_probes(tacaw_ctx *ctx, const double *probe_xy_A, int nprobes, double alpha_rad,
+                      void *d_waves, void *stream);
+
+/* O5-O7 multislice ("FFTs (the core of the multislice computations)", :92, :122;
+ * z-segments :72-84, :231).  For every wave w, with f = wave_frame[w]:
+ *   psi <- IFFT2{ P M FFT2{ t_n psi } }  for all slices of segment 0, then segment 1, ...
+ *   P[h,k] = exp(-i pi lambda dz q^2),  M = band-limit mask of the context.
+ * d_waves     DEVICE complex64 [nwaves][ny][nx], overwritten with the exit waves.
+ * d_probes    DEVICE complex64 [.][ny][nx] or NULL.  NULL: d_waves holds the entrance waves.
+ *             Non-NULL: wave w starts from d_probes[wave_probe[w]] (d_waves is output only).
+ * wave_probe  HOST int32 [nwaves] (ignored when d_probes is NULL)
+ * wave_frame  HOST int32 [nwaves], values in [0, nframes_in_flight); waves that share a frame
+ *             should be adjacent (they then share each t_n read).
+ * d_trans     HOST array [nframes_in_flight*nsegments] of DEVICE pointers;
+ *             d_trans[f*nsegments+k] -> complex64 [nslices_per_segment[k]][ny][nx]
+ * output_space 0: r-space psi_S;  1: q-space Psi_S = FFT2(psi_S), unnormalised, native FFT order. */
+int tacaw_propagate(tacaw_ctx *ctx, void *d_waves, const void *d_probes, const int32_t *wave_probe,
+                    const int32_t *wave_frame, int nwaves, const void *const *d_trans,
+                    int nframes_in_flight, const int32_t *nslices_per_segment, int nsegments,
+                    double slice_thickness_A, int output_space, void *stream);
+
+/* O8 ROI map, HOST, exact: enumerate k = -ny/2..ny/2-1 (outer),
+ * h = -nx/2..nx/2-1 (inner), keep by predicate, emit the native flat FFT index
+ * ((k+ny)%ny)*nx + (h+nx)%nx.  idx_out NULL: count only. */
+int tacaw_make_roi(const tacaw_grid *grid, double lambda_A, int mode, const double *params_rad,
+                   int32_t *idx_out, int64_t *count);
+
+/* a6 on-the-fly gather ("collects the time-consecutive exit wave functions from the
+ * defined ROI", :132):  buf[p][f][r] = Psi_S(w)[roi_idx[r]] / sqrt(nx ny),  p = wave_probe[w],
+ * f = wave_frame[w].
+ * d_qwaves  DEVICE complex64 [nwaves][ny][nx] (q-space output of tacaw_propagate)
+ * wave_probe, wave_frame  HOST int32 [nwaves] (frame = index on the time axis of d_buf)
+ * d_roi_idx DEVICE int32 [nroi]
+ * d_buf     DEVICE complex64 [nprobes][nframes][nroi]  (time-ordered buffer; r fastest) */
+int tacaw_accumulate(tacaw_ctx *ctx, const void *d_qwaves, int nwaves, const int32_t *wave_probe,
+                     const int32_t *wave_frame, const int32_t *d_roi_idx, int64_t nroi, void *d_buf,
+                     int nprobes, int nframes, void *stream);
+
+/* O9-O10 spectrum (Eq.(1) :37; :122, :142):
+ *   Phi_k = sum_f w_f buf[p][f][r] exp(-2 pi i k f/T);  E_k = h k'/(T dt), k' = k or k-T
+ *   I[p][e][r] = B(E_e/(k_B T_K)) |Phi|^2 / (T sum_f w_f^2),  B(x) = x/(1-exp(-x)), B(0) = 1
+ * Energies ascending, restricted to [emin_meV, emax_meV] (inclusive, 1e-9 meV slack).
+ * nframes: power of two in [8, 2048].
+ * d_I HOST-NULLABLE: pass d_I = NULL to query nE / the axis only.
+ * d_I      DEVICE float [nprobes][nE][nroi];  E_axis_meV_out HOST double [>= nE] or NULL; nE HOST. */
+int tacaw_spectrum(tacaw_ctx *ctx, const void *d_buf, int nprobes, int64_t nroi, int nframes, double dt_fs,
+                   int window, double temperature_K, double emin_meV, double emax_meV, float *d_I,
+                   double *E_axis_meV_out, int *nE, void *stream);
+
+/* Convenience for host-resident data (bench.py's end-to-end leg): same as the calls above but the
+ * named buffers are HOST memory; the library stages them through its own device scratch with
+ * cudaMemcpyAsync on `stream` and synchronises before returning. */
+int tacaw_build_slices_host(tacaw_ctx *ctx, const double *h_pos_A, const int32_t *h_species, int natoms,
+                            const tacaw_species *species, double slice_thickness_A, int nslices, double z0_A,
+                            void *d_trans, int *n_clamped, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TACAW_H */

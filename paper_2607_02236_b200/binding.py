@@ -1,0 +1,238 @@
+"""Thin Python binding of libtacaw.so (include/tacaw.h): argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels; PyTorch is used for device memory and
+streams.  There is no CPU fallback: if the shared library is missing or there is no CUDA device the
+calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import List, Optional, Sequence, Tuple
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libtacaw.so")
+
+EXPORTS = ["tacaw_version", "tacaw_create", "tacaw_destroy", "tacaw_last_error", "tacaw_launch_count",
+           "tacaw_build_slices", "tacaw_build_slices_host", "tacaw_make_probes", "tacaw_propagate",
+           "tacaw_make_roi", "tacaw_accumulate", "tacaw_spectrum"]
+
+ROI_MODES = {"full": 0, "disc": 1, "annulus": 2, "rect": 3}
+
+
+class TacawError(RuntimeError):
+    pass
+
+
+class _Grid(C.Structure):
+    _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("lx_A", C.c_double), ("ly_A", C.c_double)]
+
+
+class _Beam(C.Structure):
+    _fields_ = [("lambda_A", C.c_double), ("sigma_rad_per_VA", C.c_double), ("bandlimit", C.c_int)]
+
+
+class _Species(C.Structure):
+    _fields_ = [("nspecies", C.c_int), ("a", C.c_void_p), ("b", C.c_void_p)]
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen libtacaw.so; raises TacawError if it has not been built (no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise TacawError(f"{LIB_PATH} not found: build it with `python -m paper_2607_02236_b200.build` "
+                             "(or __graft_entry__.build()); there is no CPU fallback")
+        lib = C.CDLL(LIB_PATH)
+        lib.tacaw_version.restype = C.c_char_p
+        lib.tacaw_last_error.restype = C.c_char_p
+        lib.tacaw_last_error.argtypes = [C.c_void_p]
+        lib.tacaw_launch_count.restype = C.c_int64
+        lib.tacaw_launch_count.argtypes = [C.c_void_p]
+        _lib = lib
+    return _lib
+
+
+def make_roi(nx: int, ny: int, lx: float, ly: float, lam: float, mode: str, params_rad: Sequence[float]) -> np.ndarray:
+    """tacaw_make_roi (host, exact): int32 flat FFT indices in ascending (k, h) order."""
+    lib = load_library()
+    g = _Grid(nx, ny, lx, ly)
+    params = (C.c_double * 4)(*(list(params_rad) + [0.0] * 4)[:4])
+    cnt = C.c_int64(0)
+    rc = lib.tacaw_make_roi(C.byref(g), C.c_double(lam), C.c_int(ROI_MODES[mode]), params, None, C.byref(cnt))
+    if rc != 0:
+        raise TacawError(f"tacaw_make_roi failed ({rc})")
+    idx = np.empty(cnt.value, dtype=np.int32)
+    rc = lib.tacaw_make_roi(C.byref(g), C.c_double(lam), C.c_int(ROI_MODES[mode]), params,
+                            idx.ctypes.data_as(C.c_void_p), C.byref(cnt))
+    if rc != 0:
+        raise TacawError(f"tacaw_make_roi failed ({rc})")
+    return idx
+
+
+def _i32(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+class Tacaw:
+    """One context = one grid + beam on one CUDA device (tacaw_create / tacaw_destroy)."""
+
+    def __init__(self, nx: int, ny: int, lx: float, ly: float, lam: float, sigma: float, bandlimit: int = 1,
+                 device: int = 0):
+        import torch
+        self.torch = torch
+        if not torch.cuda.is_available():
+            raise TacawError("no CUDA device: the TACAW path has no CPU fallback")
+        self.lib = load_library()
+        self.nx, self.ny, self.lx, self.ly, self.lam, self.sigma = nx, ny, lx, ly, lam, sigma
+        self.device = device
+        self._ctx = C.c_void_p()
+        g, b = _Grid(nx, ny, lx, ly), _Beam(lam, sigma, bandlimit)
+        rc = self.lib.tacaw_create(C.byref(self._ctx), C.byref(g), C.byref(b), C.c_int(device))
+        if rc != 0:
+            raise TacawError(f"tacaw_create failed ({rc})")
+
+    def close(self):
+        if getattr(self, "_ctx", None) is not None and self._ctx.value:
+            self.lib.tacaw_destroy(self._ctx)
+            self._ctx = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ------------------------------------------------------------------------------------------
+    def _check(self, rc: int, what: str):
+        if rc != 0:
+            msg = self.lib.tacaw_last_error(self._ctx)
+            raise TacawError(f"{what} failed ({rc}): {msg.decode() if msg else ''}")
+
+    def _stream(self) -> C.c_void_p:
+        return C.c_void_p(self.torch.cuda.current_stream(self.device).cuda_stream)
+
+    def _dev(self, t, dtype, what):
+        if not (t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+            raise TacawError(f"{what}: need a contiguous CUDA tensor of dtype {dtype}")
+        return C.c_void_p(t.data_ptr())
+
+    @property
+    def launches(self) -> int:
+        return int(self.lib.tacaw_launch_count(self._ctx))
+
+    def _species(self, a, b):
+        a = np.ascontiguousarray(a, dtype=np.float64)
+        b = np.ascontiguousarray(b, dtype=np.float64)
+        return _Species(a.shape[0], a.ctypes.data, b.ctypes.data), (a, b)
+
+    # ------------------------------------------------------------------------------------------
+    def build_slices(self, pos, species, a, b, dz: float, nslices: int, z0: float = 0.0, out=None,
+                     want_clamped: bool = False):
+        """tacaw_build_slices.  pos: CUDA float64 [Na][3]; species: CUDA int32 [Na].
+        Returns (trans complex64 [S][ny][nx], n_clamped or None)."""
+        torch = self.torch
+        if out is None:
+            out = torch.empty((nslices, self.ny, self.nx), dtype=torch.complex64, device=pos.device)
+        sp, keep = self._species(a, b)
+        ncl = C.c_int(0)
+        rc = self.lib.tacaw_build_slices(self._ctx, self._dev(pos, torch.float64, "pos"),
+                                         self._dev(species, torch.int32, "species"), C.c_int(pos.shape[0]), C.byref(sp),
+                                         C.c_double(dz), C.c_int(nslices), C.c_double(z0),
+                                         self._dev(out, torch.complex64, "trans"),
+                                         C.byref(ncl) if want_clamped else None, self._stream())
+        self._check(rc, "tacaw_build_slices")
+        return out, (int(ncl.value) if want_clamped else None)
+
+    def build_slices_host(self, pos_h: np.ndarray, species_h: np.ndarray, a, b, dz: float, nslices: int,
+                          z0: float, out):
+        """tacaw_build_slices_host: positions/species are HOST arrays (H2D inside the call)."""
+        torch = self.torch
+        pos_h = np.ascontiguousarray(pos_h, dtype=np.float64)
+        species_h = np.ascontiguousarray(species_h, dtype=np.int32)
+        sp, keep = self._species(a, b)
+        ncl = C.c_int(0)
+        rc = self.lib.tacaw_build_slices_host(self._ctx, pos_h.ctypes.data_as(C.c_void_p),
+                                              species_h.ctypes.data_as(C.c_void_p), C.c_int(pos_h.shape[0]),
+                                              C.byref(sp), C.c_double(dz), C.c_int(nslices), C.c_double(z0),
+                                              self._dev(out, torch.complex64, "trans"), C.byref(ncl), self._stream())
+        self._check(rc, "tacaw_build_slices_host")
+        return out, int(ncl.value)
+
+    def make_probes(self, probe_xy: np.ndarray, alpha_rad: float, out=None):
+        torch = self.torch
+        xy = np.ascontiguousarray(probe_xy, dtype=np.float64).reshape(-1, 2)
+        if out is None:
+            out = torch.empty((xy.shape[0], self.ny, self.nx), dtype=torch.complex64, device=f"cuda:{self.device}")
+        rc = self.lib.tacaw_make_probes(self._ctx, xy.ctypes.data_as(C.c_void_p), C.c_int(xy.shape[0]),
+                                        C.c_double(alpha_rad), self._dev(out, torch.complex64, "waves"), self._stream())
+        self._check(rc, "tacaw_make_probes")
+        return out
+
+    def propagate(self, waves, wave_frame, trans: Sequence[Sequence], dz: float, output_space: int = 1,
+                  probes=None, wave_probe=None):
+        """tacaw_propagate, in place on `waves` (CUDA complex64 [nw][ny][nx]).
+        trans[f][k]: CUDA complex64 [S_k][ny][nx] for in-flight frame f and z-segment k."""
+        torch = self.torch
+        nw = waves.shape[0]
+        nframes, nseg = len(trans), len(trans[0])
+        ptrs = (C.c_void_p * (nframes * nseg))()
+        nsl = np.array([int(t.shape[0]) for t in trans[0]], dtype=np.int32)
+        for f in range(nframes):
+            if len(trans[f]) != nseg:
+                raise TacawError("every frame needs the same number of segments")
+            for k in range(nseg):
+                t = trans[f][k]
+                if tuple(t.shape) != (int(nsl[k]), self.ny, self.nx):
+                    raise TacawError("transmission tensor has the wrong shape")
+                ptrs[f * nseg + k] = self._dev(t, torch.complex64, "trans").value
+        wf = _i32(wave_frame)
+        wp = _i32(wave_probe) if wave_probe is not None else None
+        if wf.size != nw or (wp is not None and wp.size != nw):
+            raise TacawError("wave_frame / wave_probe length mismatch")
+        if probes is not None and wp is not None and wp.size and int(wp.max()) >= probes.shape[0]:
+            raise TacawError("wave_probe out of range")
+        rc = self.lib.tacaw_propagate(self._ctx, self._dev(waves, torch.complex64, "waves"),
+                                      self._dev(probes, torch.complex64, "probes") if probes is not None else None,
+                                      wp.ctypes.data_as(C.c_void_p) if wp is not None else None,
+                                      wf.ctypes.data_as(C.c_void_p), C.c_int(nw), ptrs, C.c_int(nframes),
+                                      nsl.ctypes.data_as(C.c_void_p), C.c_int(nseg), C.c_double(dz), C.c_int(output_space),
+                                      self._stream())
+        self._check(rc, "tacaw_propagate")
+        return waves
+
+    def accumulate(self, qwaves, wave_probe, wave_frame, roi_idx, buf):
+        """tacaw_accumulate: buf (CUDA complex64 [P][T][Q]) updated in place."""
+        torch = self.torch
+        wp, wf = _i32(wave_probe), _i32(wave_frame)
+        rc = self.lib.tacaw_accumulate(self._ctx, self._dev(qwaves, torch.complex64, "qwaves"), C.c_int(qwaves.shape[0]),
+                                       wp.ctypes.data_as(C.c_void_p), wf.ctypes.data_as(C.c_void_p),
+                                       self._dev(roi_idx, torch.int32, "roi_idx"), C.c_int64(roi_idx.numel()),
+                                       self._dev(buf, torch.complex64, "buf"), C.c_int(buf.shape[0]), C.c_int(buf.shape[1]),
+                                       self._stream())
+        self._check(rc, "tacaw_accumulate")
+        return buf
+
+    def spectrum(self, buf, dt_fs: float, window: int, temperature_K: float, emin: float = -np.inf,
+                 emax: float = np.inf, out=None):
+        """tacaw_spectrum: returns (I float32 CUDA [P][nE][Q], E float64 numpy [nE])."""
+        torch = self.torch
+        P, T, Q = buf.shape
+        nE = C.c_int(0)
+        E = np.empty(T, dtype=np.float64)
+        args = [C.c_int(P), C.c_int64(Q), C.c_int(T), C.c_double(dt_fs), C.c_int(window), C.c_double(temperature_K),
+                C.c_double(emin), C.c_double(emax)]
+        rc = self.lib.tacaw_spectrum(self._ctx, None, *args, None, E.ctypes.data_as(C.c_void_p), C.byref(nE), self._stream())
+        self._check(rc, "tacaw_spectrum")
+        if out is None:
+            out = torch.empty((P, nE.value, Q), dtype=torch.float32, device=buf.device)
+        rc = self.lib.tacaw_spectrum(self._ctx, self._dev(buf, torch.complex64, "buf"), *args,
+                                     self._dev(out, torch.float32, "I"), E.ctypes.data_as(C.c_void_p), C.byref(nE),
+                                     self._stream())
+        self._check(rc, "tacaw_spectrum")
+        return out, E[: nE.value].copy()

@@ -1,0 +1,500 @@
+// api.cu -- extern "C" entry points of libtacaw (see include/tacaw.h for the contract).
+// Host logic only: argument checks, fp64 table generation, scratch management, launch order.
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+
+#include "ctx.h"
+
+namespace tacaw {
+
+int fail(tacaw_ctx* ctx, int code, const std::string& msg) {
+    if (ctx) ctx->err = msg;
+    return code;
+}
+
+int cuda_fail(tacaw_ctx* ctx, cudaError_t e, const char* where) {
+    if (ctx) ctx->err = std::string("CUDA error: ") + cudaGetErrorString(e) + " at " + where;
+    return TACAW_E_CUDA;
+}
+
+int ensure(tacaw_ctx* ctx, void** p, size_t* cur, size_t need) {
+    if (*cur >= need) return TACAW_OK;
+    // the old block may still be in use by work queued on a stream: drain before freeing
+    if (*p) {
+        cudaDeviceSynchronize();
+        cudaFree(*p);
+        *p = nullptr;
+        *cur = 0;
+    }
+    size_t sz = need + need / 4 + 256;
+    cudaError_t e = cudaMalloc(p, sz);
+    if (e != cudaSuccess) {
+        (void)cudaGetLastError();
+        return fail(ctx, TACAW_E_NOMEM, "scratch allocation failed");
+    }
+    *cur = sz;
+    return TACAW_OK;
+}
+
+static inline int sgn_index(int i, int n) { return i < n / 2 ? i : i - n; }
+
+// O5 mask predicate, restated from DESIGN.md (not shared with the oracle).
+static bool mask_in_band(int h, int k, const tacaw_grid& g) {
+    if (g.nx == g.ny && g.lx_A == g.ly_A) return 9LL * ((long long)h * h + (long long)k * k) <= (long long)g.nx * g.nx;
+    double qx = h / g.lx_A, qy = k / g.ly_A;
+    double qn = std::fmin(g.nx / (2.0 * g.lx_A), g.ny / (2.0 * g.ly_A));
+    return qx * qx + qy * qy <= (4.0 / 9.0) * qn * qn;
+}
+
+static bool supported_n(int n) { return n >= 16 && n <= 2048 && (n & (n - 1)) == 0; }
+
+static void make_roots(int n, std::vector<float2>& out) {
+    out.resize(n);
+    for (int j = 0; j < n; ++j) {
+        // exact octant symmetries are not needed at fp32: fp64 evaluation rounds correctly
+        double ang = -2.0 * M_PI * (double)j / (double)n;
+        out[j] = make_float2((float)std::cos(ang), (float)std::sin(ang));
+    }
+}
+
+static int ensure_propagator(tacaw_ctx* ctx, double dz, cudaStream_t st) {
+    if (ctx->dz_cached == dz) return TACAW_OK;
+    const tacaw_grid& g = ctx->grid;
+    std::vector<float2> px(g.nx), py(g.ny);
+    for (int ix = 0; ix < g.nx; ++ix) {
+        double h = sgn_index(ix, g.nx);
+        double ang = -M_PI * ctx->beam.lambda_A * dz * (h / g.lx_A) * (h / g.lx_A);
+        px[ix] = make_float2((float)(std::cos(ang) / g.nx), (float)(std::sin(ang) / g.nx));
+    }
+    for (int iy = 0; iy < g.ny; ++iy) {
+        double k = sgn_index(iy, g.ny);
+        double ang = -M_PI * ctx->beam.lambda_A * dz * (k / g.ly_A) * (k / g.ly_A);
+        py[iy] = make_float2((float)(std::cos(ang) / g.ny), (float)(std::sin(ang) / g.ny));
+    }
+    // tables may be in use by queued kernels of a previous dz on another stream: order on `st`
+    TACAW_CUDA(ctx, cudaStreamSynchronize(st));
+    TACAW_CUDA(ctx, cudaMemcpy(ctx->d_px, px.data(), sizeof(float2) * g.nx, cudaMemcpyHostToDevice));
+    TACAW_CUDA(ctx, cudaMemcpy(ctx->d_py, py.data(), sizeof(float2) * g.ny, cudaMemcpyHostToDevice));
+    ctx->dz_cached = dz;
+    return TACAW_OK;
+}
+
+}  // namespace tacaw
+
+using namespace tacaw;
+
+extern "C" {
+
+const char* tacaw_version(void) { return "tacaw-b200 0.1 (sm_100a)"; }
+
+const char* tacaw_last_error(const tacaw_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+int64_t tacaw_launch_count(const tacaw_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int tacaw_create(tacaw_ctx** out, const tacaw_grid* grid, const tacaw_beam* beam, int device) {
+    if (!out || !grid || !beam) return TACAW_E_ARG;
+    *out = nullptr;
+    if (!supported_n(grid->nx) || !supported_n(grid->ny)) return TACAW_E_UNSUPPORTED;
+    if (!(grid->lx_A > 0) || !(grid->ly_A > 0) || !(beam->lambda_A > 0)) return TACAW_E_ARG;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= 0 || device < 0 || device >= ndev) {
+        (void)cudaGetLastError();
+        return TACAW_E_CUDA;
+    }
+    if (cudaSetDevice(device) != cudaSuccess) return TACAW_E_CUDA;
+    tacaw_ctx* ctx = new tacaw_ctx();
+    ctx->grid = *grid;
+    ctx->beam = *beam;
+    ctx->device = device;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) == cudaSuccess) {
+        ctx->num_sms = prop.multiProcessorCount;
+        ctx->l2_bytes = (size_t)prop.l2CacheSize;
+    }
+    const int nx = grid->nx, ny = grid->ny;
+    // band-limit column extents (propagator) and potential extents (Nyquist excluded, reading G4)
+    ctx->kmax.assign(nx, -1);
+    ctx->kmax_pot.assign(nx, -1);
+    ctx->hmax = 0;
+    ctx->hmax_pot = 0;
+    ctx->kmaxmax_pot = 0;
+    for (int ix = 0; ix < nx; ++ix) {
+        int h = sgn_index(ix, nx);
+        int km = -1, kp = -1;
+        for (int k = 0; k <= ny / 2; ++k) {
+            bool in = beam->bandlimit ? mask_in_band(h, k, *grid) : true;
+            if (in) km = k;
+            if (in && 2 * k < ny && 2 * h != -nx) kp = k;
+        }
+        ctx->kmax[ix] = km;
+        ctx->kmax_pot[ix] = kp;
+        int ah = h < 0 ? -h : h;
+        if (km >= 0 && ah > ctx->hmax) ctx->hmax = ah;
+        if (kp >= 0 && ah > ctx->hmax_pot) ctx->hmax_pot = ah;
+        if (kp > ctx->kmaxmax_pot) ctx->kmaxmax_pot = kp;
+    }
+    std::vector<float2> rx, ry;
+    make_roots(nx, rx);
+    make_roots(ny, ry);
+    bool ok = cudaMalloc(&ctx->d_roots_x, sizeof(float2) * nx) == cudaSuccess &&
+              cudaMalloc(&ctx->d_roots_y, sizeof(float2) * ny) == cudaSuccess &&
+              cudaMalloc(&ctx->d_kmax, sizeof(int) * nx) == cudaSuccess &&
+              cudaMalloc(&ctx->d_kmax_pot, sizeof(int) * nx) == cudaSuccess &&
+              cudaMalloc(&ctx->d_px, sizeof(float2) * nx) == cudaSuccess &&
+              cudaMalloc(&ctx->d_py, sizeof(float2) * ny) == cudaSuccess;
+    ok = ok && cudaMemcpy(ctx->d_roots_x, rx.data(), sizeof(float2) * nx, cudaMemcpyHostToDevice) == cudaSuccess &&
+         cudaMemcpy(ctx->d_roots_y, ry.data(), sizeof(float2) * ny, cudaMemcpyHostToDevice) == cudaSuccess &&
+         cudaMemcpy(ctx->d_kmax, ctx->kmax.data(), sizeof(int) * nx, cudaMemcpyHostToDevice) == cudaSuccess &&
+         cudaMemcpy(ctx->d_kmax_pot, ctx->kmax_pot.data(), sizeof(int) * nx, cudaMemcpyHostToDevice) == cudaSuccess;
+    if (!ok) {
+        (void)cudaGetLastError();
+        tacaw_destroy(ctx);
+        return TACAW_E_CUDA;
+    }
+    *out = ctx;
+    return TACAW_OK;
+}
+
+int tacaw_destroy(tacaw_ctx* ctx) {
+    if (!ctx) return TACAW_E_ARG;
+    cudaDeviceSynchronize();
+    cudaFree(ctx->d_roots_x); cudaFree(ctx->d_roots_y); cudaFree(ctx->d_kmax); cudaFree(ctx->d_kmax_pot);
+    cudaFree(ctx->d_px); cudaFree(ctx->d_py); cudaFree(ctx->d_meta); cudaFree(ctx->d_sort); cudaFree(ctx->d_stage);
+    cudaFree(ctx->d_spec_tab);
+    (void)cudaGetLastError();
+    delete ctx;
+    return TACAW_OK;
+}
+
+int tacaw_build_slices(tacaw_ctx* ctx, const double* d_pos_A, const int32_t* d_species, int natoms,
+                       const tacaw_species* species, double dz, int nslices, double z0, void* d_trans, int* n_clamped,
+                       void* stream) {
+    if (!ctx) return TACAW_E_ARG;
+    if (natoms < 0 || nslices <= 0 || !(dz > 0) || !d_trans || !species || species->nspecies <= 0 || !species->a ||
+        !species->b || (natoms > 0 && (!d_pos_A || !d_species)))
+        return fail(ctx, TACAW_E_ARG, "tacaw_build_slices: bad argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    const int ns = species->nspecies;
+    const int nx = ctx->grid.nx, ny = ctx->grid.ny;
+    // species table -> device (float), clamp counters: meta region [ab ns*8 floats][2 ints]
+    size_t need = sizeof(float) * 8 * (size_t)ns + 2 * sizeof(int) + 64;
+    int rc = ensure(ctx, &ctx->d_meta, &ctx->meta_bytes, need > 4096 ? need : 4096);
+    if (rc) return rc;
+    std::vector<float> ab(8 * (size_t)ns);
+    for (int s = 0; s < ns; ++s)
+        for (int i = 0; i < 4; ++i) {
+            ab[8 * s + i] = (float)species->a[4 * s + i];
+            ab[8 * s + 4 + i] = (float)species->b[4 * s + i];
+        }
+    float* d_ab = (float*)ctx->d_meta;
+    int* d_ncl = (int*)((char*)ctx->d_meta + ((sizeof(float) * 8 * (size_t)ns + 15) / 16) * 16);
+    TACAW_CUDA(ctx, cudaMemcpyAsync(d_ab, ab.data(), sizeof(float) * ab.size(), cudaMemcpyHostToDevice, st));
+    rc = launch_potential(ctx, d_pos_A, d_species, natoms, ns, d_ab, dz, nslices, z0, (float2*)d_trans, d_ncl, st);
+    if (rc) return rc;
+    // V(q) -> v(r) -> t = exp(i sigma v):  IFFT_y over the in-band columns, then IFFT_x + exp per row
+    ColArgs ca{};
+    ca.waves = (float2*)d_trans; ca.nwaves = nslices; ca.nx = nx; ca.hmax = ctx->hmax_pot; ca.roots = ctx->d_roots_y;
+    ca.px = nullptr; ca.py = nullptr; ca.kmax = ctx->d_kmax_pot; ca.pscale = 1.f; ca.all_groups = 0;
+    rc = launch_col(ctx, COL_INV, ca, ny, st);
+    if (rc) return rc;
+    RowArgs ra{};
+    ra.waves = (float2*)d_trans; ra.nwaves = nslices; ra.ny = ny; ra.hmax = ctx->hmax_pot; ra.roots = ctx->d_roots_x;
+    ra.scale = (float)(ctx->beam.sigma_rad_per_VA / (ctx->grid.lx_A * ctx->grid.ly_A));
+    rc = launch_row(ctx, ROW_TRANS, ra, st);
+    if (rc) return rc;
+    int h_ncl[2] = {0, 0};
+    if (n_clamped) {
+        TACAW_CUDA(ctx, cudaMemcpyAsync(h_ncl, d_ncl, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
+        TACAW_CUDA(ctx, cudaStreamSynchronize(st));
+        *n_clamped = h_ncl[0];
+        if (h_ncl[1] > 0) return fail(ctx, TACAW_E_ARG, "tacaw_build_slices: species id out of range");
+    }
+    return TACAW_OK;
+}
+
+int tacaw_build_slices_host(tacaw_ctx* ctx, const double* h_pos_A, const int32_t* h_species, int natoms,
+                            const tacaw_species* species, double dz, int nslices, double z0, void* d_trans,
+                            int* n_clamped, void* stream) {
+    if (!ctx) return TACAW_E_ARG;
+    if (natoms < 0 || (natoms > 0 && (!h_pos_A || !h_species))) return fail(ctx, TACAW_E_ARG, "bad argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    size_t nb_pos = sizeof(double) * 3 * (size_t)natoms, nb_sp = sizeof(int32_t) * (size_t)natoms;
+    int rc = ensure(ctx, &ctx->d_stage, &ctx->stage_bytes, nb_pos + nb_sp + 64);
+    if (rc) return rc;
+    double* d_pos = (double*)ctx->d_stage;
+    int32_t* d_sp = (int32_t*)((char*)ctx->d_stage + nb_pos);
+    if (natoms > 0) {
+        TACAW_CUDA(ctx, cudaMemcpyAsync(d_pos, h_pos_A, nb_pos, cudaMemcpyHostToDevice, st));
+        TACAW_CUDA(ctx, cudaMemcpyAsync(d_sp, h_species, nb_sp, cudaMemcpyHostToDevice, st));
+    }
+    int dummy = 0;
+    rc = tacaw_build_slices(ctx, d_pos, d_sp, natoms, species, dz, nslices, z0, d_trans, n_clamped ? n_clamped : &dummy,
+                            stream);
+    return rc;
+}
+
+int tacaw_make_probes(tacaw_ctx* ctx, const double* probe_xy_A, int nprobes, double alpha_rad, void* d_waves,
+                      void* stream) {
+    if (!ctx) return TACAW_E_ARG;
+    if (nprobes < 0 || (nprobes > 0 && (!probe_xy_A || !d_waves)) || alpha_rad < 0)
+        return fail(ctx, TACAW_E_ARG, "tacaw_make_probes: bad argument");
+    if (nprobes == 0) return TACAW_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    const tacaw_grid& g = ctx->grid;
+    const int nx = g.nx, ny = g.ny;
+    // aperture decision in fp64 (O4, reading G8): A = 1 iff lambda^2 q^2 <= alpha^2
+    std::vector<int> kap(nx, -1);
+    long long n_in = 0;
+    int hap = 0;
+    const double lam = ctx->beam.lambda_A;
+    for (int ix = 0; ix < nx; ++ix) {
+        int h = sgn_index(ix, nx);
+        for (int iy = 0; iy < ny; ++iy) {
+            int k = sgn_index(iy, ny);
+            double q2 = (h / g.lx_A) * (h / g.lx_A) + (k / g.ly_A) * (k / g.ly_A);
+            if (lam * lam * q2 <= alpha_rad * alpha_rad) {
+                ++n_in;
+                int ak = k < 0 ? -k : k;
+                // the disc is symmetric except for the unpaired Nyquist index -ny/2
+                if (2 * ak < ny && ak > kap[ix]) kap[ix] = ak;
+                if (2 * ak == ny) return fail(ctx, TACAW_E_UNSUPPORTED, "aperture reaches the Nyquist frequency");
+                int ah = h < 0 ? -h : h;
+                if (ah > hap) hap = ah;
+            }
+        }
+    }
+    if (n_in == 0) return fail(ctx, TACAW_E_ARG, "empty aperture");
+    std::vector<uint32_t> uxy(2 * (size_t)nprobes);
+    for (int p = 0; p < nprobes; ++p) {
+        double fx = probe_xy_A[2 * p] / g.lx_A, fy = probe_xy_A[2 * p + 1] / g.ly_A;
+        fx -= std::floor(fx);
+        fy -= std::floor(fy);
+        uxy[2 * p] = (uint32_t)(unsigned long long)std::llrint(fx * 4294967296.0);
+        uxy[2 * p + 1] = (uint32_t)(unsigned long long)std::llrint(fy * 4294967296.0);
+    }
+    size_t need = sizeof(int) * nx + sizeof(uint32_t) * uxy.size() + 64;
+    int rc = ensure(ctx, &ctx->d_meta, &ctx->meta_bytes, need > 4096 ? need : 4096);
+    if (rc) return rc;
+    int* d_kap = (int*)ctx->d_meta;
+    uint32_t* d_uxy = (uint32_t*)(d_kap + nx);
+    TACAW_CUDA(ctx, cudaMemcpyAsync(d_kap, kap.data(), sizeof(int) * nx, cudaMemcpyHostToDevice, st));
+    TACAW_CUDA(ctx, cudaMemcpyAsync(d_uxy, uxy.data(), sizeof(uint32_t) * uxy.size(), cudaMemcpyHostToDevice, st));
+    // unit norm: the unscaled inverse transform of n_in unit phasors has sum |psi|^2 = nx ny n_in
+    float amp = (float)(1.0 / std::sqrt((double)nx * (double)ny * (double)n_in));
+    rc = launch_probe_fill(ctx, d_uxy, nprobes, d_kap, amp, (float2*)d_waves, st);
+    if (rc) return rc;
+    ColArgs ca{};
+    ca.waves = (float2*)d_waves; ca.nwaves = nprobes; ca.nx = nx; ca.hmax = hap; ca.roots = ctx->d_roots_y;
+    ca.kmax = d_kap; ca.pscale = 1.f; ca.all_groups = 0;
+    rc = launch_col(ctx, COL_INV, ca, ny, st);
+    if (rc) return rc;
+    RowArgs ra{};
+    ra.waves = (float2*)d_waves; ra.nwaves = nprobes; ra.ny = ny; ra.hmax = hap; ra.roots = ctx->d_roots_x;
+    rc = launch_row(ctx, ROW_LAST, ra, st);
+    if (rc) return rc;
+    // d_meta is reused by later calls: make sure the fill kernel has consumed it
+    TACAW_CUDA(ctx, cudaStreamSynchronize(st));
+    return TACAW_OK;
+}
+
+int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, const int32_t* wave_probe,
+                    const int32_t* wave_frame, int nwaves, const void* const* d_trans, int nframes,
+                    const int32_t* nslices_per_segment, int nsegments, double dz, int output_space, void* stream) {
+    if (!ctx) return TACAW_E_ARG;
+    if (nwaves < 0 || nframes <= 0 || nsegments <= 0 || !(dz > 0) || !d_trans || !nslices_per_segment ||
+        (nwaves > 0 && (!d_waves || !wave_frame)) || (d_probes && !wave_probe) || (output_space != 0 && output_space != 1))
+        return fail(ctx, TACAW_E_ARG, "tacaw_propagate: bad argument");
+    if (nwaves == 0) return TACAW_OK;
+    int total = 0;
+    for (int k = 0; k < nsegments; ++k) {
+        if (nslices_per_segment[k] < 0) return fail(ctx, TACAW_E_ARG, "negative slice count");
+        total += nslices_per_segment[k];
+    }
+    if (total == 0) return fail(ctx, TACAW_E_ARG, "tacaw_propagate: no slices");
+    for (int w = 0; w < nwaves; ++w) {
+        if (wave_frame[w] < 0 || wave_frame[w] >= nframes) return fail(ctx, TACAW_E_ARG, "wave_frame out of range");
+        if (d_probes && wave_probe[w] < 0) return fail(ctx, TACAW_E_ARG, "wave_probe out of range");
+    }
+    for (int i = 0; i < nframes * nsegments; ++i)
+        if (!d_trans[i] && nslices_per_segment[i % nsegments] > 0) return fail(ctx, TACAW_E_ARG, "null transmission pointer");
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = ensure_propagator(ctx, dz, st);
+    if (rc) return rc;
+    const tacaw_grid& g = ctx->grid;
+    const size_t npix = (size_t)g.nx * g.ny;
+    // metadata: [wave_frame nwaves][wave_probe nwaves][trans ptrs nframes*nseg]
+    size_t nb_i = sizeof(int) * (size_t)nwaves;
+    size_t off_p = ((2 * nb_i + 15) / 16) * 16;
+    size_t need = off_p + sizeof(void*) * (size_t)nframes * nsegments + 64;
+    rc = ensure(ctx, &ctx->d_meta, &ctx->meta_bytes, need > 4096 ? need : 4096);
+    if (rc) return rc;
+    int* d_wf = (int*)ctx->d_meta;
+    int* d_wp = d_wf + nwaves;
+    const float2** d_tp = (const float2**)((char*)ctx->d_meta + off_p);
+    TACAW_CUDA(ctx, cudaMemcpyAsync(d_wf, wave_frame, nb_i, cudaMemcpyHostToDevice, st));
+    if (d_probes) TACAW_CUDA(ctx, cudaMemcpyAsync(d_wp, wave_probe, nb_i, cudaMemcpyHostToDevice, st));
+    TACAW_CUDA(ctx, cudaMemcpyAsync((void*)d_tp, d_trans, sizeof(void*) * (size_t)nframes * nsegments, cudaMemcpyHostToDevice, st));
+
+    // depth-first over groups of waves small enough to stay L2-resident between the two kernels of
+    // a slice step: all slices for group 0, then group 1, ...
+    size_t budget = ctx->l2_bytes ? ctx->l2_bytes / 2 : (size_t)48 << 20;
+    if (const char* e = getenv("TACAW_L2_GROUP_MB")) {
+        double mb = atof(e);
+        if (mb > 0) budget = (size_t)(mb * 1048576.0);
+    }
+    int group = (int)(budget / (npix * sizeof(float2)));
+    if (group < 1) group = 1;
+    if (group > nwaves) group = nwaves;
+    for (int w0 = 0; w0 < nwaves; w0 += group) {
+        int nw = nwaves - w0 < group ? nwaves - w0 : group;
+        // do not cut a frame's run of waves in two unless the group is a single frame anyway
+        if (w0 + nw < nwaves && nw > 1) {
+            int cut = nw;
+            while (cut > 1 && wave_frame[w0 + cut] == wave_frame[w0 + cut - 1]) --cut;
+            if (cut > 1 || wave_frame[w0 + 1] != wave_frame[w0]) nw = cut;
+        }
+        int step = 0;
+        for (int k = 0; k < nsegments; ++k) {
+            for (int n = 0; n < nslices_per_segment[k]; ++n, ++step) {
+                RowArgs ra{};
+                ra.waves = (float2*)d_waves + (size_t)w0 * npix;
+                ra.probes = (step == 0) ? (const float2*)d_probes : nullptr;
+                ra.wave_probe = d_wp + w0; ra.wave_frame = d_wf + w0; ra.trans = d_tp;
+                ra.nseg = nsegments; ra.seg = k; ra.slice = n; ra.nwaves = nw; ra.ny = g.ny; ra.hmax = ctx->hmax;
+                ra.roots = ctx->d_roots_x;
+                rc = launch_row(ctx, step == 0 ? ROW_FIRST : ROW_MID, ra, st);
+                if (rc) return rc;
+                bool lastq = (step == total - 1) && output_space == 1;
+                ColArgs ca{};
+                ca.waves = ra.waves; ca.nwaves = nw; ca.nx = g.nx; ca.hmax = ctx->hmax; ca.roots = ctx->d_roots_y;
+                ca.px = ctx->d_px; ca.py = ctx->d_py; ca.kmax = ctx->d_kmax;
+                ca.pscale = lastq ? (float)((double)g.nx * (double)g.ny) : 1.f;
+                ca.all_groups = lastq ? 1 : 0;
+                rc = launch_col(ctx, lastq ? COL_LASTQ : COL_MID, ca, g.ny, st);
+                if (rc) return rc;
+            }
+        }
+        if (output_space == 0) {
+            RowArgs ra{};
+            ra.waves = (float2*)d_waves + (size_t)w0 * npix; ra.nwaves = nw; ra.ny = g.ny; ra.hmax = ctx->hmax;
+            ra.roots = ctx->d_roots_x;
+            rc = launch_row(ctx, ROW_LAST, ra, st);
+            if (rc) return rc;
+        }
+        w0 += nw - group;   // the loop adds `group`
+    }
+    return TACAW_OK;
+}
+
+int tacaw_make_roi(const tacaw_grid* g, double lambda, int mode, const double* params, int32_t* idx_out, int64_t* count) {
+    if (!g || !count || g->nx <= 0 || g->ny <= 0 || (mode != TACAW_ROI_FULL && !params)) return TACAW_E_ARG;
+    if (mode < 0 || mode > 3) return TACAW_E_ARG;
+    const bool square = (g->nx == g->ny && g->lx_A == g->ly_A);
+    int64_t c = 0;
+    for (int k = -g->ny / 2; k < g->ny - g->ny / 2; ++k)
+        for (int h = -g->nx / 2; h < g->nx - g->nx / 2; ++h) {
+            bool keep = true;
+            if (mode == TACAW_ROI_DISC || mode == TACAW_ROI_ANNULUS) {
+                double t2;
+                if (square) {
+                    double s = lambda / g->lx_A;
+                    t2 = s * s * (double)((long long)h * h + (long long)k * k);
+                } else {
+                    t2 = lambda * lambda * ((h / g->lx_A) * (h / g->lx_A) + (k / g->ly_A) * (k / g->ly_A));
+                }
+                double to = (mode == TACAW_ROI_DISC) ? params[0] : params[1];
+                keep = t2 <= to * to;
+                if (mode == TACAW_ROI_ANNULUS) keep = keep && t2 >= params[0] * params[0];
+            } else if (mode == TACAW_ROI_RECT) {
+                double tx = lambda * h / g->lx_A, ty = lambda * k / g->ly_A;
+                keep = tx >= params[0] && tx <= params[1] && ty >= params[2] && ty <= params[3];
+            }
+            if (keep) {
+                if (idx_out) idx_out[c] = (int32_t)(((k + g->ny) % g->ny) * g->nx + (h + g->nx) % g->nx);
+                ++c;
+            }
+        }
+    *count = c;
+    return TACAW_OK;
+}
+
+int tacaw_accumulate(tacaw_ctx* ctx, const void* d_qwaves, int nwaves, const int32_t* wave_probe,
+                     const int32_t* wave_frame, const int32_t* d_roi_idx, int64_t nroi, void* d_buf, int nprobes,
+                     int nframes, void* stream) {
+    if (!ctx) return TACAW_E_ARG;
+    if (nwaves < 0 || nroi < 0 || nprobes <= 0 || nframes <= 0 ||
+        (nwaves > 0 && nroi > 0 && (!d_qwaves || !wave_probe || !wave_frame || !d_roi_idx || !d_buf)))
+        return fail(ctx, TACAW_E_ARG, "tacaw_accumulate: bad argument");
+    if (nwaves == 0 || nroi == 0) return TACAW_OK;
+    for (int w = 0; w < nwaves; ++w)
+        if (wave_probe[w] < 0 || wave_probe[w] >= nprobes || wave_frame[w] < 0 || wave_frame[w] >= nframes)
+            return fail(ctx, TACAW_E_ARG, "tacaw_accumulate: probe/frame index out of range");
+    cudaStream_t st = (cudaStream_t)stream;
+    // index arrays go to the staging region (stream-ordered after any earlier user of it)
+    size_t nb_i = sizeof(int) * (size_t)nwaves;
+    size_t need = 4 * nb_i + 4096;
+    int rc = ensure(ctx, &ctx->d_stage, &ctx->stage_bytes, need);
+    if (rc) return rc;
+    int* d_wp = (int*)ctx->d_stage;
+    int* d_wf = d_wp + nwaves;
+    TACAW_CUDA(ctx, cudaMemcpyAsync(d_wp, wave_probe, nb_i, cudaMemcpyHostToDevice, st));
+    TACAW_CUDA(ctx, cudaMemcpyAsync(d_wf, wave_frame, nb_i, cudaMemcpyHostToDevice, st));
+    return launch_gather(ctx, (const float2*)d_qwaves, nwaves, d_wp, d_wf, d_roi_idx, nroi, (float2*)d_buf, nprobes,
+                         nframes, st);
+}
+
+int tacaw_spectrum(tacaw_ctx* ctx, const void* d_buf, int nprobes, int64_t nroi, int nframes, double dt_fs, int window,
+                   double temperature_K, double emin, double emax, float* d_I, double* E_out, int* nE_out, void* stream) {
+    if (!ctx) return TACAW_E_ARG;
+    if (nprobes < 0 || nroi < 0 || nframes <= 0 || !(dt_fs > 0) || !(temperature_K > 0) || !nE_out ||
+        (window != TACAW_WINDOW_RECT && window != TACAW_WINDOW_HANN))
+        return fail(ctx, TACAW_E_ARG, "tacaw_spectrum: bad argument");
+    if (nframes < 8 || nframes > 2048 || (nframes & (nframes - 1))) return fail(ctx, TACAW_E_UNSUPPORTED, "nframes must be a power of two in [8, 2048]");
+    const double h_mev_fs = 4135.667696, kb_mev = 8.617333262e-2;
+    const int T = nframes;
+    // ascending axis k' = -T/2 .. T/2-1; keep [emin, emax] with 1e-9 meV slack (reading G11)
+    int e_lo = -1, nE = 0;
+    std::vector<double> E;
+    for (int i = 0; i < T; ++i) {
+        double e = h_mev_fs * (double)(i - T / 2) / ((double)T * dt_fs);
+        if (e < emin - 1e-9 || e > emax + 1e-9) continue;
+        if (e_lo < 0) e_lo = i;
+        E.push_back(e);
+        ++nE;
+    }
+    *nE_out = nE;
+    if (E_out) for (int i = 0; i < nE; ++i) E_out[i] = E[i];
+    if (!d_I || nE == 0 || nprobes == 0 || nroi == 0) return TACAW_OK;
+    if (!d_buf) return fail(ctx, TACAW_E_ARG, "tacaw_spectrum: null buffer");
+    cudaStream_t st = (cudaStream_t)stream;
+    std::vector<float> tab(2 * (size_t)T + (size_t)T + (size_t)nE);   // roots (float2 x T), window, bose
+    double sw2 = 0.0;
+    std::vector<double> w(T);
+    for (int f = 0; f < T; ++f) {
+        w[f] = (window == TACAW_WINDOW_HANN) ? 0.5 - 0.5 * std::cos(2.0 * M_PI * (double)f / (double)T) : 1.0;
+        sw2 += w[f] * w[f];
+    }
+    for (int j = 0; j < T; ++j) {
+        double ang = -2.0 * M_PI * (double)j / (double)T;
+        tab[2 * j] = (float)std::cos(ang);
+        tab[2 * j + 1] = (float)std::sin(ang);
+        tab[2 * (size_t)T + j] = (float)w[j];
+    }
+    for (int i = 0; i < nE; ++i) {
+        double x = E[i] / (kb_mev * temperature_K);
+        double B = (x == 0.0) ? 1.0 : x / (-std::expm1(-x));
+        tab[3 * (size_t)T + i] = (float)(B / ((double)T * sw2));
+    }
+    int rc = ensure(ctx, (void**)&ctx->d_spec_tab, &ctx->spec_tab_bytes, sizeof(float) * tab.size());
+    if (rc) return rc;
+    TACAW_CUDA(ctx, cudaMemcpyAsync(ctx->d_spec_tab, tab.data(), sizeof(float) * tab.size(), cudaMemcpyHostToDevice, st));
+    rc = launch_spectrum(ctx, (const float2*)d_buf, nprobes, nroi, T, (const float2*)ctx->d_spec_tab,
+                         ctx->d_spec_tab + 2 * (size_t)T, ctx->d_spec_tab + 3 * (size_t)T, e_lo, nE, d_I, st);
+    if (rc) return rc;
+    // `tab` is a pageable host buffer: the async copy has been staged by the runtime on return
+    return TACAW_OK;
+}
+
+}  // extern "C"

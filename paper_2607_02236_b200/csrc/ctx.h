@@ -1,0 +1,101 @@
+// ctx.h -- internal context of libtacaw (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "../../include/tacaw.h"
+
+struct tacaw_ctx {
+    tacaw_grid grid{};
+    tacaw_beam beam{};
+    int device = 0;
+    int num_sms = 148;
+    size_t l2_bytes = 0;
+
+    float2* d_roots_x = nullptr;  // exp(-2 pi i j/nx), j < nx
+    float2* d_roots_y = nullptr;  // exp(-2 pi i j/ny)
+    int* d_kmax = nullptr;        // [nx] per column ix: largest |k| inside the band-limit mask, -1 = none
+    int* d_kmax_pot = nullptr;    // [nx] same for the potential (Nyquist row/column excluded)
+    std::vector<int> kmax, kmax_pot;
+    int hmax = 0;                 // largest |h| with any in-band k  (propagator mask)
+    int hmax_pot = 0;             // same for the potential
+    int kmaxmax_pot = 0;
+
+    double dz_cached = -1.0;
+    float2* d_px = nullptr;  // [nx] exp(-i pi lambda dz h^2/lx^2) / nx
+    float2* d_py = nullptr;  // [ny] exp(-i pi lambda dz k^2/ly^2) / ny
+
+    // scratch: metadata region (per-call index arrays) and sort region (build_slices)
+    void* d_meta = nullptr;
+    size_t meta_bytes = 0;
+    void* d_sort = nullptr;
+    size_t sort_bytes = 0;
+    void* d_stage = nullptr;  // staging for the *_host convenience calls
+    size_t stage_bytes = 0;
+    float* d_spec_tab = nullptr;  // window + bose tables
+    size_t spec_tab_bytes = 0;
+
+    std::string err;
+    int64_t launches = 0;
+};
+
+namespace tacaw {
+
+int fail(tacaw_ctx* ctx, int code, const std::string& msg);
+int cuda_fail(tacaw_ctx* ctx, cudaError_t e, const char* where);
+int ensure(tacaw_ctx* ctx, void** p, size_t* cur, size_t need);
+
+#define TACAW_CUDA(ctx, call)                                        \
+    do {                                                             \
+        cudaError_t e__ = (call);                                    \
+        if (e__ != cudaSuccess) return tacaw::cuda_fail(ctx, e__, #call); \
+    } while (0)
+
+// launchers implemented in the kernel translation units --------------------------------------
+enum RowMode { ROW_FIRST = 0, ROW_MID = 1, ROW_LAST = 2, ROW_TRANS = 3 };
+enum ColMode { COL_MID = 0, COL_LASTQ = 1, COL_INV = 2 };
+
+struct RowArgs {
+    float2* waves;                 // [nwaves][ny][nx]
+    const float2* probes;          // or nullptr
+    const int* wave_probe;         // device
+    const int* wave_frame;         // device
+    const float2* const* trans;    // device [nframes*nseg] segment base pointers
+    int nseg, seg, slice;          // which t_n this step uses: trans[f*nseg+seg] + slice*ny*nx
+    int nwaves, ny;
+    int hmax;                      // in-band columns: ix <= hmax || ix >= nx-hmax
+    int wpc;                       // waves per CTA
+    const float2* roots;
+    float scale;                   // ROW_TRANS: sigma/(lx ly)
+};
+
+struct ColArgs {
+    float2* waves;
+    int nwaves, nx;
+    int hmax;
+    int wpc;
+    const float2* roots;           // ny-th roots
+    const float2* px;
+    const float2* py;
+    const int* kmax;
+    float pscale;                  // multiplies px*py (1 for COL_MID, nx*ny for COL_LASTQ)
+    int all_groups;                // 1: every column group (mask ignored for group selection)
+};
+
+int launch_row(tacaw_ctx* ctx, int mode, const RowArgs& a, cudaStream_t st);
+int launch_col(tacaw_ctx* ctx, int mode, const ColArgs& a, int ny, cudaStream_t st);
+
+int launch_potential(tacaw_ctx* ctx, const double* d_pos, const int32_t* d_species, int natoms, int nspecies,
+                     const float* d_ab /*[ns][8]*/, double dz, int nslices, double z0, float2* d_V, int* d_nclamped,
+                     cudaStream_t st);
+int launch_probe_fill(tacaw_ctx* ctx, const uint32_t* d_uxy /*[P][2] fixed-point fractional*/, int nprobes,
+                      const int* d_kap /*[nx]*/, float amp, float2* d_waves, cudaStream_t st);
+int launch_gather(tacaw_ctx* ctx, const float2* d_q, int nwaves, const int* d_wp, const int* d_wf, const int* d_idx,
+                  int64_t nroi, float2* d_buf, int nprobes, int nframes, cudaStream_t st);
+int launch_spectrum(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int64_t nroi, int nframes, const float2* d_roots,
+                    const float* d_window, const float* d_bose, int e_lo, int nE, float* d_I, cudaStream_t st);
+
+}  // namespace tacaw

@@ -1,0 +1,297 @@
+// potential.cu -- slice binning (a1), structure-factor potential (K1), probe fill (K3), ROI gather (K5).
+//
+// K1 (O2):  V_n[h,k] = sum_s f_s(q^2) sum_{j in (n,s)} exp(-2 pi i (h x_j/lx + k y_j/ly)),
+// f_s(q^2) = sum_{i<4} a_si exp(-b_si q^2), on in-band (h,k) only.  The phase factorises per atom,
+// exp(-2 pi i h u_j) exp(-2 pi i k v_j), so a slice is a rank-K complex outer-product sum; each
+// CTA owns a 64 x 32 (h,k) tile, stages the per-atom phase vectors of a chunk of atoms in shared
+// memory and accumulates 4x2 outputs per thread in registers.  v_n is real, so only k >= 0 is
+// computed and V(-h,-k) = conj V(h,k) is mirrored on store.
+// Phases use fixed-point fractional coordinates U = round(u 2^32): (h*U mod 2^32) is exact
+// integer arithmetic, then sincospif -- fp32 h*x/L would lose ~4e-4 rad at |h| ~ 1000.
+#include "ctx.h"
+
+namespace tacaw {
+
+// ---------------------------------------------------------------------------------------- a1
+// key_j = slice*nspecies + species;  fixed-point fractional coordinates.
+__global__ void k_atom_keys(const double* __restrict__ pos, const int32_t* __restrict__ species, int natoms,
+                            int nspecies, double dz, int nslices, double z0, double inv_lx, double inv_ly,
+                            int* __restrict__ keys, uint32_t* __restrict__ ux, uint32_t* __restrict__ uy,
+                            int* __restrict__ counts, int* __restrict__ nclamped) {
+    int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= natoms) return;
+    double f = floor((pos[3 * (size_t)j + 2] - z0) / dz);
+    int n;
+    if (f < 0.0) { n = 0; atomicAdd(nclamped, 1); }
+    else if (f > (double)(nslices - 1)) { n = nslices - 1; atomicAdd(nclamped, 1); }
+    else n = (int)f;
+    int s = species[j];
+    if (s < 0 || s >= nspecies) { atomicAdd(nclamped + 1, 1); s = 0; }
+    int key = n * nspecies + s;
+    keys[j] = key;
+    atomicAdd(counts + key, 1);
+    double fx = pos[3 * (size_t)j] * inv_lx, fy = pos[3 * (size_t)j + 1] * inv_ly;
+    fx -= floor(fx);
+    fy -= floor(fy);
+    ux[j] = (uint32_t)(unsigned long long)llrint(fx * 4294967296.0);   // wraps 2^32 -> 0
+    uy[j] = (uint32_t)(unsigned long long)llrint(fy * 4294967296.0);
+}
+
+// exclusive scan of counts[nkeys] -> offsets[nkeys+1]; one CTA.
+__global__ void k_scan_counts(const int* __restrict__ counts, int nkeys, int* __restrict__ offsets) {
+    __shared__ int part[1024];
+    __shared__ int carry;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    for (int base = 0; base < nkeys; base += blockDim.x) {
+        int i = base + threadIdx.x;
+        int v = (i < nkeys) ? counts[i] : 0;
+        part[threadIdx.x] = v;
+        __syncthreads();
+        for (int d = 1; d < blockDim.x; d <<= 1) {
+            int t = (threadIdx.x >= d) ? part[threadIdx.x - d] : 0;
+            __syncthreads();
+            part[threadIdx.x] += t;
+            __syncthreads();
+        }
+        if (i < nkeys) offsets[i] = carry + part[threadIdx.x] - v;
+        __syncthreads();
+        if (threadIdx.x == blockDim.x - 1) carry += part[threadIdx.x];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) offsets[nkeys] = carry;
+}
+
+// One CTA per key: stable compaction (original atom order) of the atoms carrying that key.
+__global__ void k_compact(const int* __restrict__ keys, int natoms, const int* __restrict__ offsets,
+                          const uint32_t* __restrict__ ux, const uint32_t* __restrict__ uy,
+                          uint32_t* __restrict__ sx, uint32_t* __restrict__ sy) {
+    const int key = blockIdx.x;
+    const int out0 = offsets[key];
+    if (offsets[key + 1] == out0) return;
+    __shared__ int warp_tot[32];
+    __shared__ int running;
+    if (threadIdx.x == 0) running = 0;
+    __syncthreads();
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    for (int base = 0; base < natoms; base += blockDim.x) {
+        int j = base + threadIdx.x;
+        bool hit = (j < natoms) && (keys[j] == key);
+        unsigned bal = __ballot_sync(0xffffffffu, hit);
+        int rank = __popc(bal & ((1u << lane) - 1));
+        if (lane == 0) warp_tot[wid] = __popc(bal);
+        __syncthreads();
+        int before = 0;
+        for (int w = 0; w < wid; ++w) before += warp_tot[w];
+        if (hit) {
+            int o = out0 + running + before + rank;
+            sx[o] = ux[j];
+            sy[o] = uy[j];
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            int tot = 0;
+            for (int w = 0; w < nw; ++w) tot += warp_tot[w];
+            running += tot;
+        }
+        __syncthreads();
+    }
+}
+
+// ---------------------------------------------------------------------------------------- K1
+constexpr int POT_TH = 64;    // h extent of a tile
+constexpr int POT_TK = 32;    // k extent of a tile
+constexpr int POT_CHUNK = 32; // atoms staged per step
+
+__device__ __forceinline__ float2 phase_fixed(uint32_t u, int h) {
+    // exp(-2 pi i h u/2^32): (h*u mod 2^32) as a signed fraction of a half turn
+    int32_t p = (int32_t)((uint32_t)h * u);
+    float s, c;
+    sincospif((float)p * 4.656612873077393e-10f, &s, &c);   // p / 2^31
+    return make_float2(c, -s);
+}
+
+__global__ void __launch_bounds__(256) k_potential(const uint32_t* __restrict__ sx, const uint32_t* __restrict__ sy,
+                                                    const int* __restrict__ offsets, int nspecies,
+                                                    const float* __restrict__ ab /*[ns][8]: a0..a3,b0..b3*/,
+                                                    const int* __restrict__ kmax_pot, int hmax, int nx, int ny,
+                                                    float inv_lx, float inv_ly, float2* __restrict__ V) {
+    __shared__ float2 ex[POT_CHUNK][POT_TH];
+    __shared__ float2 ey[POT_CHUNK][POT_TK];
+    const int n = blockIdx.z;
+    const int h0 = -hmax + blockIdx.x * POT_TH;
+    const int k0 = blockIdx.y * POT_TK;
+    const int th = threadIdx.x & 15, tk = threadIdx.x >> 4;   // 16 x 16 threads, 4 x 2 outputs each
+    float2 acc[4][2];
+    float2 vsum[4][2];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 2; ++j) vsum[i][j] = make_float2(0.f, 0.f);
+    for (int s = 0; s < nspecies; ++s) {
+        const int a0 = offsets[n * nspecies + s], a1 = offsets[n * nspecies + s + 1];
+        if (a0 == a1) continue;
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < 2; ++j) acc[i][j] = make_float2(0.f, 0.f);
+        for (int base = a0; base < a1; base += POT_CHUNK) {
+            const int cnt = min(POT_CHUNK, a1 - base);
+            __syncthreads();
+            for (int i = threadIdx.x; i < cnt * (POT_TH + POT_TK); i += blockDim.x) {
+                int at = i / (POT_TH + POT_TK), r = i % (POT_TH + POT_TK);
+                if (r < POT_TH) ex[at][r] = phase_fixed(sx[base + at], h0 + r);
+                else ey[at][r - POT_TH] = phase_fixed(sy[base + at], k0 + r - POT_TH);
+            }
+            __syncthreads();
+            for (int at = 0; at < cnt; ++at) {
+                float2 xh[4], yk[2];
+#pragma unroll
+                for (int i = 0; i < 4; ++i) xh[i] = ex[at][th + 16 * i];
+#pragma unroll
+                for (int j = 0; j < 2; ++j) yk[j] = ey[at][tk + 16 * j];
+#pragma unroll
+                for (int i = 0; i < 4; ++i)
+#pragma unroll
+                    for (int j = 0; j < 2; ++j) {
+                        acc[i][j].x = fmaf(xh[i].x, yk[j].x, fmaf(-xh[i].y, yk[j].y, acc[i][j].x));
+                        acc[i][j].y = fmaf(xh[i].x, yk[j].y, fmaf(xh[i].y, yk[j].x, acc[i][j].y));
+                    }
+            }
+        }
+        const float* as = ab + 8 * s;
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                float qx = (float)(h0 + th + 16 * i) * inv_lx, qy = (float)(k0 + tk + 16 * j) * inv_ly;
+                float q2 = qx * qx + qy * qy;
+                float f = 0.f;
+#pragma unroll
+                for (int g = 0; g < 4; ++g) f += as[g] * expf(-as[4 + g] * q2);
+                vsum[i][j].x = fmaf(f, acc[i][j].x, vsum[i][j].x);
+                vsum[i][j].y = fmaf(f, acc[i][j].y, vsum[i][j].y);
+            }
+    }
+    float2* Vn = V + (size_t)n * nx * ny;
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+            int h = h0 + th + 16 * i, k = k0 + tk + 16 * j;
+            if (h > hmax || h < -hmax) continue;
+            int ix = (h + nx) % nx;
+            if (k > kmax_pot[ix]) continue;
+            int iy = k;
+            Vn[(size_t)iy * nx + ix] = vsum[i][j];
+            if (k > 0) {
+                int ixm = (nx - ix) % nx, iym = ny - k;
+                Vn[(size_t)iym * nx + ixm] = make_float2(vsum[i][j].x, -vsum[i][j].y);
+            }
+        }
+}
+
+int launch_potential(tacaw_ctx* ctx, const double* d_pos, const int32_t* d_species, int natoms, int nspecies,
+                     const float* d_ab, double dz, int nslices, double z0, float2* d_V, int* d_nclamped,
+                     cudaStream_t st) {
+    const int nx = ctx->grid.nx, ny = ctx->grid.ny;
+    const int nkeys = nslices * nspecies;
+    // sort scratch layout: keys[na] ux[na] uy[na] sx[na] sy[na] counts[nkeys] offsets[nkeys+1]
+    size_t na = (size_t)(natoms > 0 ? natoms : 1);
+    size_t need = sizeof(int) * (5 * na + 2 * (size_t)nkeys + 2);
+    int rc = ensure(ctx, &ctx->d_sort, &ctx->sort_bytes, need);
+    if (rc) return rc;
+    int* keys = (int*)ctx->d_sort;
+    uint32_t* ux = (uint32_t*)(keys + na);
+    uint32_t* uy = ux + na;
+    uint32_t* sx = uy + na;
+    uint32_t* sy = sx + na;
+    int* counts = (int*)(sy + na);
+    int* offsets = counts + nkeys;
+    TACAW_CUDA(ctx, cudaMemsetAsync(counts, 0, sizeof(int) * (2 * (size_t)nkeys + 1), st));
+    TACAW_CUDA(ctx, cudaMemsetAsync(d_nclamped, 0, 2 * sizeof(int), st));
+    TACAW_CUDA(ctx, cudaMemsetAsync(d_V, 0, sizeof(float2) * (size_t)nslices * nx * ny, st));
+    if (natoms > 0) {
+        k_atom_keys<<<(natoms + 255) / 256, 256, 0, st>>>(d_pos, d_species, natoms, nspecies, dz, nslices, z0,
+                                                          1.0 / ctx->grid.lx_A, 1.0 / ctx->grid.ly_A, keys, ux, uy,
+                                                          counts, d_nclamped);
+        ctx->launches++;
+    }
+    k_scan_counts<<<1, 1024, 0, st>>>(counts, nkeys, offsets);
+    ctx->launches++;
+    if (natoms > 0) {
+        k_compact<<<nkeys, 256, 0, st>>>(keys, natoms, offsets, ux, uy, sx, sy);
+        ctx->launches++;
+        const int hmax = ctx->hmax_pot;
+        dim3 grid((2 * hmax + 1 + POT_TH - 1) / POT_TH, (ctx->kmaxmax_pot + 1 + POT_TK - 1) / POT_TK, nslices);
+        k_potential<<<grid, 256, 0, st>>>(sx, sy, offsets, nspecies, d_ab, ctx->d_kmax_pot, hmax, nx, ny,
+                                          (float)(1.0 / ctx->grid.lx_A), (float)(1.0 / ctx->grid.ly_A), d_V);
+        ctx->launches++;
+    }
+    TACAW_CUDA(ctx, cudaGetLastError());
+    return TACAW_OK;
+}
+
+// ---------------------------------------------------------------------------------------- K3
+// Psi0[h,k] = amp * exp(-2 pi i (h xp/lx + k yp/ly)) inside the aperture, else 0 (q space).
+// The aperture decision (lambda^2 q^2 <= alpha^2) is taken on the host in fp64 and arrives as
+// kap[ix] = largest |k| inside the aperture for column ix (-1: none).
+__global__ void k_probe_fill(const uint32_t* __restrict__ uxy, int nx, int ny, const int* __restrict__ kap, float amp,
+                             float2* __restrict__ waves) {
+    const int p = blockIdx.y;
+    const size_t npix = (size_t)nx * ny;
+    const uint32_t ux = uxy[2 * p], uy = uxy[2 * p + 1];
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < npix; i += (size_t)gridDim.x * blockDim.x) {
+        int ix = (int)(i % nx), iy = (int)(i / nx);
+        int h = ix < nx / 2 ? ix : ix - nx, k = iy < ny / 2 ? iy : iy - ny;
+        float2 v = make_float2(0.f, 0.f);
+        if (abs(k) <= kap[ix]) {
+            float2 e = phase_fixed(ux, h), f = phase_fixed(uy, k);
+            v = make_float2(amp * (e.x * f.x - e.y * f.y), amp * (e.x * f.y + e.y * f.x));
+        }
+        waves[(size_t)p * npix + i] = v;
+    }
+}
+
+int launch_probe_fill(tacaw_ctx* ctx, const uint32_t* d_uxy, int nprobes, const int* d_kap, float amp, float2* d_waves,
+                      cudaStream_t st) {
+    const int nx = ctx->grid.nx, ny = ctx->grid.ny;
+    int bx = (int)(((size_t)nx * ny + 255) / 256);
+    if (bx > 1024) bx = 1024;
+    k_probe_fill<<<dim3(bx, nprobes), 256, 0, st>>>(d_uxy, nx, ny, d_kap, amp, d_waves);
+    ctx->launches++;
+    TACAW_CUDA(ctx, cudaGetLastError());
+    return TACAW_OK;
+}
+
+// ---------------------------------------------------------------------------------------- K5
+__global__ void k_gather(const float2* __restrict__ q, const int* __restrict__ wp, const int* __restrict__ wf,
+                         const int* __restrict__ idx, long long nroi, float2* __restrict__ buf, int nframes,
+                         size_t npix, float scale) {
+    const int w = blockIdx.y;
+    const float2* src = q + (size_t)w * npix;
+    float2* dst = buf + ((size_t)wp[w] * nframes + wf[w]) * (size_t)nroi;
+    for (long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x; r < nroi; r += (long long)gridDim.x * blockDim.x) {
+        float2 v = src[idx[r]];
+        dst[r] = make_float2(v.x * scale, v.y * scale);
+    }
+}
+
+int launch_gather(tacaw_ctx* ctx, const float2* d_q, int nwaves, const int* d_wp, const int* d_wf, const int* d_idx,
+                  int64_t nroi, float2* d_buf, int nprobes, int nframes, cudaStream_t st) {
+    (void)nprobes;
+    if (nwaves <= 0 || nroi <= 0) return TACAW_OK;
+    const size_t npix = (size_t)ctx->grid.nx * ctx->grid.ny;
+    int bx = (int)((nroi + 255) / 256);
+    if (bx > 64) bx = 64;
+    for (int w0 = 0; w0 < nwaves; w0 += 32768) {
+        int nw = nwaves - w0 < 32768 ? nwaves - w0 : 32768;
+        k_gather<<<dim3(bx, nw), 256, 0, st>>>(d_q + (size_t)w0 * npix, d_wp + w0, d_wf + w0, d_idx, (long long)nroi, d_buf,
+                                               nframes, npix, (float)(1.0 / sqrt((double)npix)));
+        ctx->launches++;
+    }
+    TACAW_CUDA(ctx, cudaGetLastError());
+    return TACAW_OK;
+}
+
+}  // namespace tacaw

@@ -1,0 +1,107 @@
+// spectrum.cu -- K6: window x batched time FFT x |.|^2 x Bose/detailed-balance factor.
+//
+//   Phi_k = sum_f w_f buf[p][f][r] exp(-2 pi i k f/T)                     (O9, O10)
+//   I[p][e][r] = B(E_e/kBT) |Phi_k|^2 / (T sum w^2),  energies ascending, cropped to the E-ROI
+// buf is [P][T][Q] (r fastest), so a CTA takes a [T x WQ] tile -- the same vector-FFT machinery as
+// the multislice column kernel: thread (tid, c) holds frames tid + Tt*m of series r0+c, the
+// transform leaves it with bins tid + Tt*m, which it scales and stores.  The window and the
+// per-energy factor bose[e] = B(E_e/kBT)/(T sum w^2) are fp64-computed host tables.
+#include "ctx.h"
+#include "fft_core.cuh"
+
+namespace tacaw {
+
+template <int N>
+struct SpecCfg {
+    static constexpr int E = (N >= 1024) ? 16 : 8;
+    static constexpr int T = N / E;
+    static constexpr int WQ = (N >= 512) ? 4 : 8;
+    static constexpr int THREADS = T * WQ;
+    static constexpr bool TWREG = (E == 8);
+};
+
+template <int N>
+__global__ void __launch_bounds__(SpecCfg<N>::THREADS) k_spectrum(const float2* __restrict__ buf, long long nroi,
+                                                                  const float2* __restrict__ roots,
+                                                                  const float* __restrict__ window,
+                                                                  const float* __restrict__ bose, int e_lo, int nE,
+                                                                  float* __restrict__ I) {
+    using C = SpecCfg<N>;
+    constexpr int E = C::E, T = C::T, WQ = C::WQ;
+    constexpr bool TWREG = C::TWREG;
+    using P = FftPlan<N, E>;
+    extern __shared__ float2 smem[];
+    const int lt = threadIdx.x;
+    const int c = lt % WQ, tid = lt / WQ;
+    float2* smA = smem;
+    float2* smB = smem + (size_t)N * WQ;
+    const float2* roots_s = nullptr;
+    float2 tw[P::NTW];
+    if constexpr (TWREG) {
+        TwInit<N, E, 1, 0>::run(tw, roots, tid);
+    } else {
+        float2* rs = smem + (size_t)2 * N * WQ;
+        for (int i = lt; i < N; i += blockDim.x) rs[i] = roots[i];
+        roots_s = rs;
+        __syncthreads();
+    }
+    const int p = blockIdx.y;
+    const long long r = (long long)blockIdx.x * WQ + c;
+    const bool live = r < nroi;
+    const float2* src = buf + (size_t)p * N * (size_t)nroi + (live ? r : 0);
+    float2 x[E];
+#pragma unroll
+    for (int m = 0; m < E; ++m) {
+        int f = tid + T * m;
+        float2 v = live ? src[(size_t)f * nroi] : make_float2(0.f, 0.f);
+        float w = window[f];
+        x[m] = make_float2(v.x * w, v.y * w);
+    }
+    if constexpr (C::THREADS <= 32) fft_regs<N, E, WQ, false, TWREG>(x, tw, roots_s, smA, smB, tid, c, SyncWarp{});
+    else fft_regs<N, E, WQ, false, TWREG>(x, tw, roots_s, smA, smB, tid, c, SyncBlock{});
+    if (!live) return;
+    float* dst = I + (size_t)p * nE * (size_t)nroi + r;
+#pragma unroll
+    for (int m = 0; m < E; ++m) {
+        int kbin = tid + T * m;
+        int e = ((kbin + N / 2) & (N - 1)) - e_lo;      // position on the ascending energy axis
+        if (e >= 0 && e < nE) dst[(size_t)e * nroi] = bose[e] * (x[m].x * x[m].x + x[m].y * x[m].y);
+    }
+}
+
+template <int N>
+static int launch_spec_n(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int64_t nroi, const float2* roots,
+                         const float* d_window, const float* d_bose, int e_lo, int nE, float* d_I, cudaStream_t st) {
+    using C = SpecCfg<N>;
+    size_t smem = (size_t)2 * N * C::WQ * sizeof(float2) + (C::TWREG ? 0 : (size_t)N * sizeof(float2));
+    auto kern = k_spectrum<N>;
+    if (smem > 48 * 1024) TACAW_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int64_t gx = (nroi + C::WQ - 1) / C::WQ;
+    for (int p0 = 0; p0 < nprobes; p0 += 32768) {
+        int np = nprobes - p0 < 32768 ? nprobes - p0 : 32768;
+        kern<<<dim3((unsigned)gx, np), C::THREADS, smem, st>>>(d_buf + (size_t)p0 * N * (size_t)nroi, (long long)nroi, roots,
+                                                              d_window, d_bose, e_lo, nE,
+                                                              d_I + (size_t)p0 * nE * (size_t)nroi);
+        ctx->launches++;
+    }
+    TACAW_CUDA(ctx, cudaGetLastError());
+    return TACAW_OK;
+}
+
+int launch_spectrum(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int64_t nroi, int nframes, const float2* d_roots,
+                    const float* d_window, const float* d_bose, int e_lo, int nE, float* d_I, cudaStream_t st) {
+    switch (nframes) {
+        case 8: return launch_spec_n<8>(ctx, d_buf, nprobes, nroi, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+        case 16: return launch_spec_n<16>(ctx, d_buf, nprobes, nroi, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+        case 32: return launch_spec_n<32>(ctx, d_buf, nprobes, nroi, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+        case 64: return launch_spec_n<64>(ctx, d_buf, nprobes, nroi, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+        case 128: return launch_spec_n<128>(ctx, d_buf, nprobes, nroi, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+        case 256: return launch_spec_n<256>(ctx, d_buf, nprobes, nroi, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+        case 512: return launch_spec_n<512>(ctx, d_buf, nprobes, nroi, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+        case 1024: return launch_spec_n<1024>(ctx, d_buf, nprobes, nroi, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+        case 2048: return launch_spec_n<2048>(ctx, d_buf, nprobes, nroi, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+    }
+    return fail(ctx, TACAW_E_UNSUPPORTED, "nframes must be a power of two in [8, 2048]");
+}
+
+}  // namespace tacaw

@@ -209,9 +209,12 @@ def _raster(x0: float, y0: float, wx: float, wy: float, npx: int, npy: int) -> n
     return np.stack([xx.ravel(), yy.ravel()], axis=1)
 
 
-def make_workload(cfg: int, *, nframes: int | None = None, nprobes: int | None = None) -> Workload:
+def make_workload(cfg: int, *, nframes: int | None = None, nprobes: int | None = None,
+                  ncz: int | None = None) -> Workload:
     """configs[cfg-1] of BASELINE.json (cfg = 1..5).  `nframes` / `nprobes` only *truncate* the
-    workload (first frames / first probes) for sampled parity and bounded benchmarks."""
+    workload (first frames / first probes) for sampled parity and bounded benchmarks; `ncz`
+    (cells along z, per segment) makes a thinner sample of the same lateral size and grid for
+    parity cases the fp64 oracle can finish."""
     a0, c0 = RUTILE_A, RUTILE_C
     dz = 0.5 * c0
     kv = 100.0
@@ -240,7 +243,7 @@ def make_workload(cfg: int, *, nframes: int | None = None, nprobes: int | None =
         wl = Workload("c2", n, n, ncx * a0, ncy * a0, kv, lam, sig, 30.0, probes, T, dt, temp, dz,
                       [seg], "disc", (60.0,), sa, sb)
     elif cfg == 3:
-        ncx, ncy, ncz, n, T, dt = 10, 10, 100, 512, 1024, 5.0
+        ncx, ncy, ncz, n, T, dt = 10, 10, (ncz or 100), 512, 1024, 5.0
         pos0, spec = rutile_supercell(ncx, ncy, ncz)
         rng = np.random.default_rng(SEED_BASE + 100 * cfg)
         ms = _mode_set(rng, 64, 0.0, 110.0, ncx * a0, ncy * a0, ncz * c0, "thermal", temp)
@@ -249,7 +252,7 @@ def make_workload(cfg: int, *, nframes: int | None = None, nprobes: int | None =
         wl = Workload("c3", n, n, ncx * a0, ncy * a0, kv, lam, sig, 30.0, probes, T, dt, temp, dz,
                       [seg], "disc", (40.0,), sa, sb)
     elif cfg == 4:
-        ncx, ncy, ncz_seg, nseg, n, T, dt = 12, 12, 85, 4, 1024, 1024, 5.0
+        ncx, ncy, ncz_seg, nseg, n, T, dt = 12, 12, (ncz or 85), 4, 1024, 1024, 5.0
         segs = []
         for k in range(nseg):
             pos0, spec = rutile_supercell(ncx, ncy, ncz_seg)
@@ -260,7 +263,7 @@ def make_workload(cfg: int, *, nframes: int | None = None, nprobes: int | None =
         wl = Workload("c4", n, n, ncx * a0, ncy * a0, kv, lam, sig, 30.0, probes, T, dt, temp, dz,
                       segs, "disc", (50.0,), sa, sb)
     elif cfg == 5:
-        ncx, ncy, ncz, n, T, dt = 24, 24, 60, 2048, 2048, 4.0
+        ncx, ncy, ncz, n, T, dt = 24, 24, (ncz or 60), 2048, 2048, 4.0
         pos0, spec = rutile_supercell(ncx, ncy, ncz)
         lx = ncx * a0
         shift = pos0[:, 0] >= 0.5 * lx           # planar fault across (100), reading G16
