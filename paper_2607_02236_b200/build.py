@@ -52,7 +52,7 @@ def build_lib(force: bool = False, verbose: bool = False) -> str:
         for l in logs:
             sys.stderr.write(l)
     tmp = LIB + f".tmp{os.getpid()}"
-    subprocess.check_call([nvcc, "-shared", "-cudart", "static", "-o", tmp, *objs])
+    subprocess.check_call([nvcc, "-shared", "-cudart", "static", "-gencode", "arch=compute_100a,code=sm_100a", "-o", tmp, *objs])
     os.replace(tmp, LIB)
     return LIB
 

@@ -38,6 +38,29 @@ int ensure(tacaw_ctx* ctx, void** p, size_t* cur, size_t need) {
     return TACAW_OK;
 }
 
+int upload(tacaw_ctx* ctx, void* dst, const void* src, size_t bytes, cudaStream_t st) {
+    if (bytes == 0) return TACAW_OK;
+    if (!ctx->h_arena) {
+        if (cudaMallocHost((void**)&ctx->h_arena, (size_t)4 << 20) == cudaSuccess) ctx->arena_bytes = (size_t)4 << 20;
+        else (void)cudaGetLastError();
+    }
+    size_t need = (bytes + 63) / 64 * 64;
+    if (need > ctx->arena_bytes) {   // pageable copy: staged by the runtime before it returns
+        TACAW_CUDA(ctx, cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, st));
+        return TACAW_OK;
+    }
+    if (ctx->arena_off + need > ctx->arena_bytes) {
+        // wrap: every copy issued from the arena so far must have completed
+        TACAW_CUDA(ctx, cudaDeviceSynchronize());
+        ctx->arena_off = 0;
+    }
+    char* h = ctx->h_arena + ctx->arena_off;
+    ctx->arena_off += need;
+    memcpy(h, src, bytes);
+    TACAW_CUDA(ctx, cudaMemcpyAsync(dst, h, bytes, cudaMemcpyHostToDevice, st));
+    return TACAW_OK;
+}
+
 static inline int sgn_index(int i, int n) { return i < n / 2 ? i : i - n; }
 
 // O5 mask predicate, restated from DESIGN.md (not shared with the oracle).
@@ -163,6 +186,7 @@ int tacaw_destroy(tacaw_ctx* ctx) {
     cudaFree(ctx->d_roots_x); cudaFree(ctx->d_roots_y); cudaFree(ctx->d_kmax); cudaFree(ctx->d_kmax_pot);
     cudaFree(ctx->d_px); cudaFree(ctx->d_py); cudaFree(ctx->d_meta); cudaFree(ctx->d_sort); cudaFree(ctx->d_stage);
     cudaFree(ctx->d_spec_tab);
+    if (ctx->h_arena) cudaFreeHost(ctx->h_arena);
     (void)cudaGetLastError();
     delete ctx;
     return TACAW_OK;
@@ -178,20 +202,17 @@ int tacaw_build_slices(tacaw_ctx* ctx, const double* d_pos_A, const int32_t* d_s
     cudaStream_t st = (cudaStream_t)stream;
     const int ns = species->nspecies;
     const int nx = ctx->grid.nx, ny = ctx->grid.ny;
-    // species table -> device (float), clamp counters: meta region [ab ns*8 floats][2 ints]
-    size_t need = sizeof(float) * 8 * (size_t)ns + 2 * sizeof(int) + 64;
-    int rc = ensure(ctx, &ctx->d_meta, &ctx->meta_bytes, need > 4096 ? need : 4096);
+    if (ns > MAX_SPECIES) return fail(ctx, TACAW_E_UNSUPPORTED, "tacaw_build_slices: at most 8 species");
+    int rc = ensure(ctx, &ctx->d_meta, &ctx->meta_bytes, 4096);
     if (rc) return rc;
-    std::vector<float> ab(8 * (size_t)ns);
+    AbTable ab{};
     for (int s = 0; s < ns; ++s)
         for (int i = 0; i < 4; ++i) {
-            ab[8 * s + i] = (float)species->a[4 * s + i];
-            ab[8 * s + 4 + i] = (float)species->b[4 * s + i];
+            ab.a[s][i] = (float)species->a[4 * s + i];
+            ab.b[s][i] = (float)species->b[4 * s + i];
         }
-    float* d_ab = (float*)ctx->d_meta;
-    int* d_ncl = (int*)((char*)ctx->d_meta + ((sizeof(float) * 8 * (size_t)ns + 15) / 16) * 16);
-    TACAW_CUDA(ctx, cudaMemcpyAsync(d_ab, ab.data(), sizeof(float) * ab.size(), cudaMemcpyHostToDevice, st));
-    rc = launch_potential(ctx, d_pos_A, d_species, natoms, ns, d_ab, dz, nslices, z0, (float2*)d_trans, d_ncl, st);
+    int* d_ncl = (int*)ctx->d_meta;   // [0] clamped atoms, [1] bad species ids
+    rc = launch_potential(ctx, d_pos_A, d_species, natoms, ns, ab, dz, nslices, z0, (float2*)d_trans, d_ncl, st);
     if (rc) return rc;
     // V(q) -> v(r) -> t = exp(i sigma v):  IFFT_y over the in-band columns, then IFFT_x + exp per row
     ColArgs ca{};
@@ -279,8 +300,8 @@ int tacaw_make_probes(tacaw_ctx* ctx, const double* probe_xy_A, int nprobes, dou
     if (rc) return rc;
     int* d_kap = (int*)ctx->d_meta;
     uint32_t* d_uxy = (uint32_t*)(d_kap + nx);
-    TACAW_CUDA(ctx, cudaMemcpyAsync(d_kap, kap.data(), sizeof(int) * nx, cudaMemcpyHostToDevice, st));
-    TACAW_CUDA(ctx, cudaMemcpyAsync(d_uxy, uxy.data(), sizeof(uint32_t) * uxy.size(), cudaMemcpyHostToDevice, st));
+    if ((rc = upload(ctx, d_kap, kap.data(), sizeof(int) * nx, st))) return rc;
+    if ((rc = upload(ctx, d_uxy, uxy.data(), sizeof(uint32_t) * uxy.size(), st))) return rc;
     // unit norm: the unscaled inverse transform of n_in unit phasors has sum |psi|^2 = nx ny n_in
     float amp = (float)(1.0 / std::sqrt((double)nx * (double)ny * (double)n_in));
     rc = launch_probe_fill(ctx, d_uxy, nprobes, d_kap, amp, (float2*)d_waves, st);
@@ -333,9 +354,9 @@ int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, const i
     int* d_wf = (int*)ctx->d_meta;
     int* d_wp = d_wf + nwaves;
     const float2** d_tp = (const float2**)((char*)ctx->d_meta + off_p);
-    TACAW_CUDA(ctx, cudaMemcpyAsync(d_wf, wave_frame, nb_i, cudaMemcpyHostToDevice, st));
-    if (d_probes) TACAW_CUDA(ctx, cudaMemcpyAsync(d_wp, wave_probe, nb_i, cudaMemcpyHostToDevice, st));
-    TACAW_CUDA(ctx, cudaMemcpyAsync((void*)d_tp, d_trans, sizeof(void*) * (size_t)nframes * nsegments, cudaMemcpyHostToDevice, st));
+    if ((rc = upload(ctx, d_wf, wave_frame, nb_i, st))) return rc;
+    if (d_probes && (rc = upload(ctx, d_wp, wave_probe, nb_i, st))) return rc;
+    if ((rc = upload(ctx, (void*)d_tp, d_trans, sizeof(void*) * (size_t)nframes * nsegments, st))) return rc;
 
     // depth-first over groups of waves small enough to stay L2-resident between the two kernels of
     // a slice step: all slices for group 0, then group 1, ...
@@ -439,8 +460,8 @@ int tacaw_accumulate(tacaw_ctx* ctx, const void* d_qwaves, int nwaves, const int
     if (rc) return rc;
     int* d_wp = (int*)ctx->d_stage;
     int* d_wf = d_wp + nwaves;
-    TACAW_CUDA(ctx, cudaMemcpyAsync(d_wp, wave_probe, nb_i, cudaMemcpyHostToDevice, st));
-    TACAW_CUDA(ctx, cudaMemcpyAsync(d_wf, wave_frame, nb_i, cudaMemcpyHostToDevice, st));
+    if ((rc = upload(ctx, d_wp, wave_probe, nb_i, st))) return rc;
+    if ((rc = upload(ctx, d_wf, wave_frame, nb_i, st))) return rc;
     return launch_gather(ctx, (const float2*)d_qwaves, nwaves, d_wp, d_wf, d_roi_idx, nroi, (float2*)d_buf, nprobes,
                          nframes, st);
 }
@@ -489,11 +510,10 @@ int tacaw_spectrum(tacaw_ctx* ctx, const void* d_buf, int nprobes, int64_t nroi,
     }
     int rc = ensure(ctx, (void**)&ctx->d_spec_tab, &ctx->spec_tab_bytes, sizeof(float) * tab.size());
     if (rc) return rc;
-    TACAW_CUDA(ctx, cudaMemcpyAsync(ctx->d_spec_tab, tab.data(), sizeof(float) * tab.size(), cudaMemcpyHostToDevice, st));
+    if ((rc = upload(ctx, ctx->d_spec_tab, tab.data(), sizeof(float) * tab.size(), st))) return rc;
     rc = launch_spectrum(ctx, (const float2*)d_buf, nprobes, nroi, T, (const float2*)ctx->d_spec_tab,
                          ctx->d_spec_tab + 2 * (size_t)T, ctx->d_spec_tab + 3 * (size_t)T, e_lo, nE, d_I, st);
     if (rc) return rc;
-    // `tab` is a pageable host buffer: the async copy has been staged by the runtime on return
     return TACAW_OK;
 }
 

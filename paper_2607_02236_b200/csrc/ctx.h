@@ -38,6 +38,11 @@ struct tacaw_ctx {
     float* d_spec_tab = nullptr;  // window + bose tables
     size_t spec_tab_bytes = 0;
 
+    // pinned host arena for per-call index arrays: lets cudaMemcpyAsync return without draining
+    // the stream (a pageable source would synchronise it)
+    char* h_arena = nullptr;
+    size_t arena_bytes = 0, arena_off = 0;
+
     std::string err;
     int64_t launches = 0;
 };
@@ -47,6 +52,14 @@ namespace tacaw {
 int fail(tacaw_ctx* ctx, int code, const std::string& msg);
 int cuda_fail(tacaw_ctx* ctx, cudaError_t e, const char* where);
 int ensure(tacaw_ctx* ctx, void** p, size_t* cur, size_t need);
+// async H2D of a small host array through the pinned arena (falls back to a pageable copy)
+int upload(tacaw_ctx* ctx, void* dst, const void* src, size_t bytes, cudaStream_t st);
+
+constexpr int MAX_SPECIES = 8;
+struct AbTable {
+    float a[MAX_SPECIES][4];
+    float b[MAX_SPECIES][4];
+};
 
 #define TACAW_CUDA(ctx, call)                                        \
     do {                                                             \
@@ -89,7 +102,7 @@ int launch_row(tacaw_ctx* ctx, int mode, const RowArgs& a, cudaStream_t st);
 int launch_col(tacaw_ctx* ctx, int mode, const ColArgs& a, int ny, cudaStream_t st);
 
 int launch_potential(tacaw_ctx* ctx, const double* d_pos, const int32_t* d_species, int natoms, int nspecies,
-                     const float* d_ab /*[ns][8]*/, double dz, int nslices, double z0, float2* d_V, int* d_nclamped,
+                     const AbTable& ab, double dz, int nslices, double z0, float2* d_V, int* d_nclamped,
                      cudaStream_t st);
 int launch_probe_fill(tacaw_ctx* ctx, const uint32_t* d_uxy /*[P][2] fixed-point fractional*/, int nprobes,
                       const int* d_kap /*[nx]*/, float amp, float2* d_waves, cudaStream_t st);

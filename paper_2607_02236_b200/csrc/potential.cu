@@ -113,7 +113,7 @@ __device__ __forceinline__ float2 phase_fixed(uint32_t u, int h) {
 
 __global__ void __launch_bounds__(256) k_potential(const uint32_t* __restrict__ sx, const uint32_t* __restrict__ sy,
                                                     const int* __restrict__ offsets, int nspecies,
-                                                    const float* __restrict__ ab /*[ns][8]: a0..a3,b0..b3*/,
+                                                    const AbTable ab,
                                                     const int* __restrict__ kmax_pot, int hmax, int nx, int ny,
                                                     float inv_lx, float inv_ly, float2* __restrict__ V) {
     __shared__ float2 ex[POT_CHUNK][POT_TH];
@@ -159,7 +159,6 @@ __global__ void __launch_bounds__(256) k_potential(const uint32_t* __restrict__ 
                     }
             }
         }
-        const float* as = ab + 8 * s;
 #pragma unroll
         for (int i = 0; i < 4; ++i)
 #pragma unroll
@@ -168,7 +167,7 @@ __global__ void __launch_bounds__(256) k_potential(const uint32_t* __restrict__ 
                 float q2 = qx * qx + qy * qy;
                 float f = 0.f;
 #pragma unroll
-                for (int g = 0; g < 4; ++g) f += as[g] * expf(-as[4 + g] * q2);
+                for (int g = 0; g < 4; ++g) f += ab.a[s][g] * expf(-ab.b[s][g] * q2);
                 vsum[i][j].x = fmaf(f, acc[i][j].x, vsum[i][j].x);
                 vsum[i][j].y = fmaf(f, acc[i][j].y, vsum[i][j].y);
             }
@@ -192,7 +191,7 @@ __global__ void __launch_bounds__(256) k_potential(const uint32_t* __restrict__ 
 }
 
 int launch_potential(tacaw_ctx* ctx, const double* d_pos, const int32_t* d_species, int natoms, int nspecies,
-                     const float* d_ab, double dz, int nslices, double z0, float2* d_V, int* d_nclamped,
+                     const AbTable& ab, double dz, int nslices, double z0, float2* d_V, int* d_nclamped,
                      cudaStream_t st) {
     const int nx = ctx->grid.nx, ny = ctx->grid.ny;
     const int nkeys = nslices * nspecies;
@@ -224,7 +223,7 @@ int launch_potential(tacaw_ctx* ctx, const double* d_pos, const int32_t* d_speci
         ctx->launches++;
         const int hmax = ctx->hmax_pot;
         dim3 grid((2 * hmax + 1 + POT_TH - 1) / POT_TH, (ctx->kmaxmax_pot + 1 + POT_TK - 1) / POT_TK, nslices);
-        k_potential<<<grid, 256, 0, st>>>(sx, sy, offsets, nspecies, d_ab, ctx->d_kmax_pot, hmax, nx, ny,
+        k_potential<<<grid, 256, 0, st>>>(sx, sy, offsets, nspecies, ab, ctx->d_kmax_pot, hmax, nx, ny,
                                           (float)(1.0 / ctx->grid.lx_A), (float)(1.0 / ctx->grid.ly_A), d_V);
         ctx->launches++;
     }
