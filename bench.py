@@ -251,15 +251,13 @@ def main():
     e2e = None
     if not args.no_e2e:
         I_host = torch.empty(I.shape, dtype=I.dtype).pin_memory()
-        h2d = sum(p.nbytes for p in pos_h) + sum(s.nbytes for s in spec_h) * wl.nframes
+        h2d = sum(p.nbytes for p in pos_h) + sum(s.nbytes for s in spec_h) * ((wl.nframes + r.fpb - 1) // r.fpb)
         d2h = I_host.numel() * 4
 
         def e2e_step():
             for f0 in range(0, wl.nframes, r.fpb):
                 nf = min(r.fpb, wl.nframes - f0)
-                for i in range(nf):
-                    for k, seg in enumerate(wl.segments):
-                        r.tc.build_slices_host(pos_h[k][f0 + i], spec_h[k], wl.a, wl.b, wl.dz, seg.nslices, 0.0, r.trans[i][k])
+                r.build_block_host(pos_h, f0, nf)
                 _, wp, wf = r.propagate_block(nf, 1)
                 r.gather_block(nf, f0, wp, wf)
             Ie, _ = r.spectrum()

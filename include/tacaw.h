@@ -82,10 +82,13 @@ int64_t tacaw_launch_count(const tacaw_ctx *ctx);
  *         clamped to the first/last slice and counted -- never wrapped, :219)
  *   V_n[h,k] = sum_{j in n} f_s(q^2) exp(-2 pi i (h x_j/lx + k y_j/ly))   on in-band (h,k)
  *   v_n = Re{ IFFT2(V_n) nx ny/(lx ly) },   t_n = exp(i sigma v_n)
- * d_pos_A   DEVICE double [natoms][3] (Angstrom);  d_species DEVICE int32 [natoms] in [0,nspecies)
- * d_trans   DEVICE complex64 [nslices][ny][nx], written
- * n_clamped HOST, optional; when non-NULL the call synchronises the stream before returning. */
-int tacaw_build_slices(tacaw_ctx *ctx, const double *d_pos_A, const int32_t *d_species, int natoms,
+ * The call is batched over MD frames (same atoms, one position set per frame):
+ * d_pos_A   DEVICE double [nframes][natoms][3] (Angstrom)
+ * d_species DEVICE int32 [natoms] in [0,nspecies), nspecies <= 8
+ * d_trans   DEVICE complex64 [nframes][nslices][ny][nx], written
+ * n_clamped HOST, optional (total over the frames); when non-NULL the call synchronises the stream
+ *           before returning. */
+int tacaw_build_slices(tacaw_ctx *ctx, const double *d_pos_A, const int32_t *d_species, int natoms, int nframes,
                        const tacaw_species *species, double slice_thickness_A, int nslices, double z0_A,
                        void *d_trans, int *n_clamped, void *stream);
 
@@ -144,7 +147,7 @@ int tacaw_spectrum(tacaw_ctx *ctx, const void *d_buf, int nprobes, int64_t nroi,
 /* Convenience for host-resident data (bench.py's end-to-end leg): same as the calls above but the
  * named buffers are HOST memory; the library stages them through its own device scratch with
  * cudaMemcpyAsync on `stream` and synchronises before returning. */
-int tacaw_build_slices_host(tacaw_ctx *ctx, const double *h_pos_A, const int32_t *h_species, int natoms,
+int tacaw_build_slices_host(tacaw_ctx *ctx, const double *h_pos_A, const int32_t *h_species, int natoms, int nframes,
                             const tacaw_species *species, double slice_thickness_A, int nslices, double z0_A,
                             void *d_trans, int *n_clamped, void *stream);
 

@@ -134,16 +134,22 @@ class Tacaw:
     # ------------------------------------------------------------------------------------------
     def build_slices(self, pos, species, a, b, dz: float, nslices: int, z0: float = 0.0, out=None,
                      want_clamped: bool = False):
-        """tacaw_build_slices.  pos: CUDA float64 [Na][3]; species: CUDA int32 [Na].
-        Returns (trans complex64 [S][ny][nx], n_clamped or None)."""
+        """tacaw_build_slices, batched over frames.  pos: CUDA float64 [F][Na][3] (or [Na][3] for one frame);
+        species: CUDA int32 [Na].  Returns (trans complex64 [F][S][ny][nx] (or [S][ny][nx]), n_clamped or None)."""
         torch = self.torch
+        single = pos.dim() == 2
+        nframes = 1 if single else int(pos.shape[0])
+        natoms = int(pos.shape[-2])
         if out is None:
-            out = torch.empty((nslices, self.ny, self.nx), dtype=torch.complex64, device=pos.device)
+            shape = (nslices, self.ny, self.nx) if single else (nframes, nslices, self.ny, self.nx)
+            out = torch.empty(shape, dtype=torch.complex64, device=pos.device)
+        if out.numel() != nframes * nslices * self.ny * self.nx:
+            raise TacawError("build_slices: output tensor has the wrong size")
         sp, keep = self._species(a, b)
         ncl = C.c_int(0)
         rc = self.lib.tacaw_build_slices(self._ctx, self._dev(pos, torch.float64, "pos"),
-                                         self._dev(species, torch.int32, "species"), C.c_int(pos.shape[0]), C.byref(sp),
-                                         C.c_double(dz), C.c_int(nslices), C.c_double(z0),
+                                         self._dev(species, torch.int32, "species"), C.c_int(natoms), C.c_int(nframes),
+                                         C.byref(sp), C.c_double(dz), C.c_int(nslices), C.c_double(z0),
                                          self._dev(out, torch.complex64, "trans"),
                                          C.byref(ncl) if want_clamped else None, self._stream())
         self._check(rc, "tacaw_build_slices")
@@ -151,14 +157,18 @@ class Tacaw:
 
     def build_slices_host(self, pos_h: np.ndarray, species_h: np.ndarray, a, b, dz: float, nslices: int,
                           z0: float, out):
-        """tacaw_build_slices_host: positions/species are HOST arrays (H2D inside the call)."""
+        """tacaw_build_slices_host: positions [F][Na][3] / species are HOST arrays (H2D inside the call)."""
         torch = self.torch
         pos_h = np.ascontiguousarray(pos_h, dtype=np.float64)
         species_h = np.ascontiguousarray(species_h, dtype=np.int32)
+        nframes = 1 if pos_h.ndim == 2 else int(pos_h.shape[0])
+        natoms = int(pos_h.shape[-2])
+        if out.numel() != nframes * nslices * self.ny * self.nx:
+            raise TacawError("build_slices_host: output tensor has the wrong size")
         sp, keep = self._species(a, b)
         ncl = C.c_int(0)
         rc = self.lib.tacaw_build_slices_host(self._ctx, pos_h.ctypes.data_as(C.c_void_p),
-                                              species_h.ctypes.data_as(C.c_void_p), C.c_int(pos_h.shape[0]),
+                                              species_h.ctypes.data_as(C.c_void_p), C.c_int(natoms), C.c_int(nframes),
                                               C.byref(sp), C.c_double(dz), C.c_int(nslices), C.c_double(z0),
                                               self._dev(out, torch.complex64, "trans"), C.byref(ncl), self._stream())
         self._check(rc, "tacaw_build_slices_host")

@@ -192,11 +192,12 @@ int tacaw_destroy(tacaw_ctx* ctx) {
     return TACAW_OK;
 }
 
-int tacaw_build_slices(tacaw_ctx* ctx, const double* d_pos_A, const int32_t* d_species, int natoms,
+int tacaw_build_slices(tacaw_ctx* ctx, const double* d_pos_A, const int32_t* d_species, int natoms, int nframes,
                        const tacaw_species* species, double dz, int nslices, double z0, void* d_trans, int* n_clamped,
                        void* stream) {
     if (!ctx) return TACAW_E_ARG;
-    if (natoms < 0 || nslices <= 0 || !(dz > 0) || !d_trans || !species || species->nspecies <= 0 || !species->a ||
+    if (nframes == 0) { if (n_clamped) *n_clamped = 0; return TACAW_OK; }
+    if (natoms < 0 || nframes < 0 || nslices <= 0 || !(dz > 0) || !d_trans || !species || species->nspecies <= 0 || !species->a ||
         !species->b || (natoms > 0 && (!d_pos_A || !d_species)))
         return fail(ctx, TACAW_E_ARG, "tacaw_build_slices: bad argument");
     cudaStream_t st = (cudaStream_t)stream;
@@ -212,16 +213,16 @@ int tacaw_build_slices(tacaw_ctx* ctx, const double* d_pos_A, const int32_t* d_s
             ab.b[s][i] = (float)species->b[4 * s + i];
         }
     int* d_ncl = (int*)ctx->d_meta;   // [0] clamped atoms, [1] bad species ids
-    rc = launch_potential(ctx, d_pos_A, d_species, natoms, ns, ab, dz, nslices, z0, (float2*)d_trans, d_ncl, st);
+    rc = launch_potential(ctx, d_pos_A, d_species, natoms, nframes, ns, ab, dz, nslices, z0, (float2*)d_trans, d_ncl, st);
     if (rc) return rc;
     // V(q) -> v(r) -> t = exp(i sigma v):  IFFT_y over the in-band columns, then IFFT_x + exp per row
     ColArgs ca{};
-    ca.waves = (float2*)d_trans; ca.nwaves = nslices; ca.nx = nx; ca.hmax = ctx->hmax_pot; ca.roots = ctx->d_roots_y;
+    ca.waves = (float2*)d_trans; ca.nwaves = nframes * nslices; ca.nx = nx; ca.hmax = ctx->hmax_pot; ca.roots = ctx->d_roots_y;
     ca.px = nullptr; ca.py = nullptr; ca.kmax = ctx->d_kmax_pot; ca.pscale = 1.f; ca.all_groups = 0;
     rc = launch_col(ctx, COL_INV, ca, ny, st);
     if (rc) return rc;
     RowArgs ra{};
-    ra.waves = (float2*)d_trans; ra.nwaves = nslices; ra.ny = ny; ra.hmax = ctx->hmax_pot; ra.roots = ctx->d_roots_x;
+    ra.waves = (float2*)d_trans; ra.nwaves = nframes * nslices; ra.ny = ny; ra.hmax = ctx->hmax_pot; ra.roots = ctx->d_roots_x;
     ra.scale = (float)(ctx->beam.sigma_rad_per_VA / (ctx->grid.lx_A * ctx->grid.ly_A));
     rc = launch_row(ctx, ROW_TRANS, ra, st);
     if (rc) return rc;
@@ -235,23 +236,23 @@ int tacaw_build_slices(tacaw_ctx* ctx, const double* d_pos_A, const int32_t* d_s
     return TACAW_OK;
 }
 
-int tacaw_build_slices_host(tacaw_ctx* ctx, const double* h_pos_A, const int32_t* h_species, int natoms,
+int tacaw_build_slices_host(tacaw_ctx* ctx, const double* h_pos_A, const int32_t* h_species, int natoms, int nframes,
                             const tacaw_species* species, double dz, int nslices, double z0, void* d_trans,
                             int* n_clamped, void* stream) {
     if (!ctx) return TACAW_E_ARG;
-    if (natoms < 0 || (natoms > 0 && (!h_pos_A || !h_species))) return fail(ctx, TACAW_E_ARG, "bad argument");
+    if (natoms < 0 || nframes < 0 || (natoms > 0 && nframes > 0 && (!h_pos_A || !h_species))) return fail(ctx, TACAW_E_ARG, "bad argument");
     cudaStream_t st = (cudaStream_t)stream;
-    size_t nb_pos = sizeof(double) * 3 * (size_t)natoms, nb_sp = sizeof(int32_t) * (size_t)natoms;
+    size_t nb_pos = sizeof(double) * 3 * (size_t)natoms * (size_t)nframes, nb_sp = sizeof(int32_t) * (size_t)natoms;
     int rc = ensure(ctx, &ctx->d_stage, &ctx->stage_bytes, nb_pos + nb_sp + 64);
     if (rc) return rc;
     double* d_pos = (double*)ctx->d_stage;
     int32_t* d_sp = (int32_t*)((char*)ctx->d_stage + nb_pos);
-    if (natoms > 0) {
+    if (natoms > 0 && nframes > 0) {
         TACAW_CUDA(ctx, cudaMemcpyAsync(d_pos, h_pos_A, nb_pos, cudaMemcpyHostToDevice, st));
         TACAW_CUDA(ctx, cudaMemcpyAsync(d_sp, h_species, nb_sp, cudaMemcpyHostToDevice, st));
     }
     int dummy = 0;
-    rc = tacaw_build_slices(ctx, d_pos, d_sp, natoms, species, dz, nslices, z0, d_trans, n_clamped ? n_clamped : &dummy,
+    rc = tacaw_build_slices(ctx, d_pos, d_sp, natoms, nframes, species, dz, nslices, z0, d_trans, n_clamped ? n_clamped : &dummy,
                             stream);
     return rc;
 }
@@ -365,17 +366,24 @@ int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, const i
         double mb = atof(e);
         if (mb > 0) budget = (size_t)(mb * 1048576.0);
     }
-    int group = (int)(budget / (npix * sizeof(float2)));
-    if (group < 1) group = 1;
-    if (group > nwaves) group = nwaves;
-    for (int w0 = 0; w0 < nwaves; w0 += group) {
-        int nw = nwaves - w0 < group ? nwaves - w0 : group;
-        // do not cut a frame's run of waves in two unless the group is a single frame anyway
-        if (w0 + nw < nwaves && nw > 1) {
-            int cut = nw;
-            while (cut > 1 && wave_frame[w0 + cut] == wave_frame[w0 + cut - 1]) --cut;
-            if (cut > 1 || wave_frame[w0 + 1] != wave_frame[w0]) nw = cut;
+    int gmax = (int)(budget / (npix * sizeof(float2)));
+    if (gmax < 1) gmax = 1;
+    const int ngroups = (nwaves + gmax - 1) / gmax;
+    int w0 = 0;
+    for (int gi = 0; gi < ngroups; ++gi) {
+        // balanced groups; a boundary moves to the nearest frame change within a quarter group
+        int w1 = (int)(((long long)(gi + 1) * nwaves) / ngroups);
+        if (gi + 1 < ngroups) {
+            const int slack = (w1 - w0) / 4;
+            for (int d = 0; d <= slack; ++d) {
+                if (w1 + d < nwaves && wave_frame[w1 + d] != wave_frame[w1 + d - 1]) { w1 += d; break; }
+                if (w1 - d > w0 && wave_frame[w1 - d] != wave_frame[w1 - d - 1]) { w1 -= d; break; }
+            }
+        } else {
+            w1 = nwaves;
         }
+        const int nw = w1 - w0;
+        if (nw <= 0) continue;
         int step = 0;
         for (int k = 0; k < nsegments; ++k) {
             for (int n = 0; n < nslices_per_segment[k]; ++n, ++step) {
@@ -404,7 +412,7 @@ int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, const i
             rc = launch_row(ctx, ROW_LAST, ra, st);
             if (rc) return rc;
         }
-        w0 += nw - group;   // the loop adds `group`
+        w0 = w1;
     }
     return TACAW_OK;
 }

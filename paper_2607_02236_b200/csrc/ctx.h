@@ -101,7 +101,7 @@ struct ColArgs {
 int launch_row(tacaw_ctx* ctx, int mode, const RowArgs& a, cudaStream_t st);
 int launch_col(tacaw_ctx* ctx, int mode, const ColArgs& a, int ny, cudaStream_t st);
 
-int launch_potential(tacaw_ctx* ctx, const double* d_pos, const int32_t* d_species, int natoms, int nspecies,
+int launch_potential(tacaw_ctx* ctx, const double* d_pos, const int32_t* d_species, int natoms, int nframes, int nspecies,
                      const AbTable& ab, double dz, int nslices, double z0, float2* d_V, int* d_nclamped,
                      cudaStream_t st);
 int launch_probe_fill(tacaw_ctx* ctx, const uint32_t* d_uxy /*[P][2] fixed-point fractional*/, int nprobes,

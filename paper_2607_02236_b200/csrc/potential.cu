@@ -13,88 +13,100 @@
 namespace tacaw {
 
 // ---------------------------------------------------------------------------------------- a1
-// key_j = slice*nspecies + species;  fixed-point fractional coordinates.
+// key_j = (frame*nslices + slice)*nspecies + species;  fixed-point fractional coordinates.
 __global__ void k_atom_keys(const double* __restrict__ pos, const int32_t* __restrict__ species, int natoms,
-                            int nspecies, double dz, int nslices, double z0, double inv_lx, double inv_ly,
-                            int* __restrict__ keys, uint32_t* __restrict__ ux, uint32_t* __restrict__ uy,
+                            long long ntotal, int nspecies, double dz, int nslices, double z0, double inv_lx,
+                            double inv_ly, int* __restrict__ keys, uint32_t* __restrict__ ux, uint32_t* __restrict__ uy,
                             int* __restrict__ counts, int* __restrict__ nclamped) {
-    int j = blockIdx.x * blockDim.x + threadIdx.x;
-    if (j >= natoms) return;
-    double f = floor((pos[3 * (size_t)j + 2] - z0) / dz);
+    long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= ntotal) return;
+    const int f = (int)(i / natoms), j = (int)(i - (long long)f * natoms);
+    double fz = floor((pos[3 * i + 2] - z0) / dz);
     int n;
-    if (f < 0.0) { n = 0; atomicAdd(nclamped, 1); }
-    else if (f > (double)(nslices - 1)) { n = nslices - 1; atomicAdd(nclamped, 1); }
-    else n = (int)f;
+    if (fz < 0.0) { n = 0; atomicAdd(nclamped, 1); }
+    else if (fz > (double)(nslices - 1)) { n = nslices - 1; atomicAdd(nclamped, 1); }
+    else n = (int)fz;
     int s = species[j];
     if (s < 0 || s >= nspecies) { atomicAdd(nclamped + 1, 1); s = 0; }
-    int key = n * nspecies + s;
-    keys[j] = key;
+    int key = (f * nslices + n) * nspecies + s;
+    keys[i] = key;
     atomicAdd(counts + key, 1);
-    double fx = pos[3 * (size_t)j] * inv_lx, fy = pos[3 * (size_t)j + 1] * inv_ly;
+    double fx = pos[3 * i] * inv_lx, fy = pos[3 * i + 1] * inv_ly;
     fx -= floor(fx);
     fy -= floor(fy);
-    ux[j] = (uint32_t)(unsigned long long)llrint(fx * 4294967296.0);   // wraps 2^32 -> 0
-    uy[j] = (uint32_t)(unsigned long long)llrint(fy * 4294967296.0);
+    ux[i] = (uint32_t)(unsigned long long)llrint(fx * 4294967296.0);   // wraps 2^32 -> 0
+    uy[i] = (uint32_t)(unsigned long long)llrint(fy * 4294967296.0);
 }
 
 // exclusive scan of counts[nkeys] -> offsets[nkeys+1]; one CTA.
 __global__ void k_scan_counts(const int* __restrict__ counts, int nkeys, int* __restrict__ offsets) {
-    __shared__ int part[1024];
+    __shared__ int warp_sum[32];
     __shared__ int carry;
     if (threadIdx.x == 0) carry = 0;
     __syncthreads();
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
     for (int base = 0; base < nkeys; base += blockDim.x) {
         int i = base + threadIdx.x;
         int v = (i < nkeys) ? counts[i] : 0;
-        part[threadIdx.x] = v;
-        __syncthreads();
-        for (int d = 1; d < blockDim.x; d <<= 1) {
-            int t = (threadIdx.x >= d) ? part[threadIdx.x - d] : 0;
-            __syncthreads();
-            part[threadIdx.x] += t;
-            __syncthreads();
+        int incl = v;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            int t = __shfl_up_sync(0xffffffffu, incl, d);
+            if (lane >= d) incl += t;
         }
-        if (i < nkeys) offsets[i] = carry + part[threadIdx.x] - v;
+        if (lane == 31) warp_sum[wid] = incl;
         __syncthreads();
-        if (threadIdx.x == blockDim.x - 1) carry += part[threadIdx.x];
+        if (wid == 0) {
+            int ws = (lane < nw) ? warp_sum[lane] : 0;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                int t = __shfl_up_sync(0xffffffffu, ws, d);
+                if (lane >= d) ws += t;
+            }
+            warp_sum[lane] = ws;     // inclusive over warps
+        }
+        __syncthreads();
+        int before = (wid > 0 ? warp_sum[wid - 1] : 0) + carry;
+        if (i < nkeys) offsets[i] = before + incl - v;
+        __syncthreads();
+        if (threadIdx.x == 0) carry += warp_sum[nw - 1];
         __syncthreads();
     }
     if (threadIdx.x == 0) offsets[nkeys] = carry;
 }
 
-// One CTA per key: stable compaction (original atom order) of the atoms carrying that key.
-__global__ void k_compact(const int* __restrict__ keys, int natoms, const int* __restrict__ offsets,
-                          const uint32_t* __restrict__ ux, const uint32_t* __restrict__ uy,
-                          uint32_t* __restrict__ sx, uint32_t* __restrict__ sy) {
-    const int key = blockIdx.x;
+// One warp per key: stable compaction (original atom order) of the atoms of that key's frame.
+__global__ void k_compact(const int* __restrict__ keys, int natoms, int nkeys_per_frame, int nkeys_total,
+                          const int* __restrict__ offsets, const uint32_t* __restrict__ ux,
+                          const uint32_t* __restrict__ uy, uint32_t* __restrict__ sx, uint32_t* __restrict__ sy) {
+    const int key = (int)(((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5);
+    const int lane = threadIdx.x & 31;
+    if (key >= nkeys_total) return;
     const int out0 = offsets[key];
-    if (offsets[key + 1] == out0) return;
-    __shared__ int warp_tot[32];
-    __shared__ int running;
-    if (threadIdx.x == 0) running = 0;
-    __syncthreads();
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
-    for (int base = 0; base < natoms; base += blockDim.x) {
-        int j = base + threadIdx.x;
-        bool hit = (j < natoms) && (keys[j] == key);
-        unsigned bal = __ballot_sync(0xffffffffu, hit);
-        int rank = __popc(bal & ((1u << lane) - 1));
-        if (lane == 0) warp_tot[wid] = __popc(bal);
-        __syncthreads();
-        int before = 0;
-        for (int w = 0; w < wid; ++w) before += warp_tot[w];
-        if (hit) {
-            int o = out0 + running + before + rank;
-            sx[o] = ux[j];
-            sy[o] = uy[j];
+    const int cnt = offsets[key + 1] - out0;
+    if (cnt == 0) return;
+    const int f = key / nkeys_per_frame;
+    const size_t fbase = (size_t)f * natoms;
+    const int* kf = keys + fbase;
+    int written = 0;
+    for (int base = 0; base < natoms && written < cnt; base += 128) {
+        int jj[4];
+        bool hit[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            jj[u] = base + 32 * u + lane;
+            hit[u] = (jj[u] < natoms) && (kf[jj[u]] == key);
         }
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            int tot = 0;
-            for (int w = 0; w < nw; ++w) tot += warp_tot[w];
-            running += tot;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            unsigned bal = __ballot_sync(0xffffffffu, hit[u]);
+            if (hit[u]) {
+                int o = out0 + written + __popc(bal & ((1u << lane) - 1));
+                sx[o] = ux[fbase + jj[u]];
+                sy[o] = uy[fbase + jj[u]];
+            }
+            written += __popc(bal);
         }
-        __syncthreads();
     }
 }
 
@@ -190,42 +202,51 @@ __global__ void __launch_bounds__(256) k_potential(const uint32_t* __restrict__ 
         }
 }
 
-int launch_potential(tacaw_ctx* ctx, const double* d_pos, const int32_t* d_species, int natoms, int nspecies,
+int launch_potential(tacaw_ctx* ctx, const double* d_pos, const int32_t* d_species, int natoms, int nframes, int nspecies,
                      const AbTable& ab, double dz, int nslices, double z0, float2* d_V, int* d_nclamped,
                      cudaStream_t st) {
     const int nx = ctx->grid.nx, ny = ctx->grid.ny;
-    const int nkeys = nslices * nspecies;
-    // sort scratch layout: keys[na] ux[na] uy[na] sx[na] sy[na] counts[nkeys] offsets[nkeys+1]
-    size_t na = (size_t)(natoms > 0 ? natoms : 1);
-    size_t need = sizeof(int) * (5 * na + 2 * (size_t)nkeys + 2);
+    const long long ntotal = (long long)natoms * nframes;
+    const long long nkeys_ll = (long long)nframes * nslices * nspecies;
+    if (nkeys_ll > (1LL << 30) || ntotal > (1LL << 31) - 1) return fail(ctx, TACAW_E_UNSUPPORTED, "batch too large");
+    const int nkeys = (int)nkeys_ll;
+    // sort scratch layout: keys[nt] ux[nt] uy[nt] sx[nt] sy[nt] counts[nkeys] offsets[nkeys+1]
+    size_t nt = (size_t)(ntotal > 0 ? ntotal : 1);
+    size_t need = sizeof(int) * (5 * nt + 2 * (size_t)nkeys + 2);
     int rc = ensure(ctx, &ctx->d_sort, &ctx->sort_bytes, need);
     if (rc) return rc;
     int* keys = (int*)ctx->d_sort;
-    uint32_t* ux = (uint32_t*)(keys + na);
-    uint32_t* uy = ux + na;
-    uint32_t* sx = uy + na;
-    uint32_t* sy = sx + na;
-    int* counts = (int*)(sy + na);
+    uint32_t* ux = (uint32_t*)(keys + nt);
+    uint32_t* uy = ux + nt;
+    uint32_t* sx = uy + nt;
+    uint32_t* sy = sx + nt;
+    int* counts = (int*)(sy + nt);
     int* offsets = counts + nkeys;
     TACAW_CUDA(ctx, cudaMemsetAsync(counts, 0, sizeof(int) * (2 * (size_t)nkeys + 1), st));
     TACAW_CUDA(ctx, cudaMemsetAsync(d_nclamped, 0, 2 * sizeof(int), st));
-    TACAW_CUDA(ctx, cudaMemsetAsync(d_V, 0, sizeof(float2) * (size_t)nslices * nx * ny, st));
-    if (natoms > 0) {
-        k_atom_keys<<<(natoms + 255) / 256, 256, 0, st>>>(d_pos, d_species, natoms, nspecies, dz, nslices, z0,
-                                                          1.0 / ctx->grid.lx_A, 1.0 / ctx->grid.ly_A, keys, ux, uy,
-                                                          counts, d_nclamped);
+    TACAW_CUDA(ctx, cudaMemsetAsync(d_V, 0, sizeof(float2) * (size_t)nframes * nslices * nx * ny, st));
+    if (ntotal > 0) {
+        k_atom_keys<<<(unsigned)((ntotal + 255) / 256), 256, 0, st>>>(d_pos, d_species, natoms, ntotal, nspecies, dz, nslices,
+                                                                     z0, 1.0 / ctx->grid.lx_A, 1.0 / ctx->grid.ly_A, keys, ux,
+                                                                     uy, counts, d_nclamped);
         ctx->launches++;
     }
     k_scan_counts<<<1, 1024, 0, st>>>(counts, nkeys, offsets);
     ctx->launches++;
-    if (natoms > 0) {
-        k_compact<<<nkeys, 256, 0, st>>>(keys, natoms, offsets, ux, uy, sx, sy);
+    if (ntotal > 0) {
+        k_compact<<<(unsigned)(((long long)nkeys * 32 + 255) / 256), 256, 0, st>>>(keys, natoms, nslices * nspecies, nkeys, offsets,
+                                                                                  ux, uy, sx, sy);
         ctx->launches++;
         const int hmax = ctx->hmax_pot;
-        dim3 grid((2 * hmax + 1 + POT_TH - 1) / POT_TH, (ctx->kmaxmax_pot + 1 + POT_TK - 1) / POT_TK, nslices);
-        k_potential<<<grid, 256, 0, st>>>(sx, sy, offsets, nspecies, ab, ctx->d_kmax_pot, hmax, nx, ny,
-                                          (float)(1.0 / ctx->grid.lx_A), (float)(1.0 / ctx->grid.ly_A), d_V);
-        ctx->launches++;
+        const int total_slices = nframes * nslices;
+        for (int z0i = 0; z0i < total_slices; z0i += 65535) {
+            int nz = total_slices - z0i < 65535 ? total_slices - z0i : 65535;
+            dim3 grid((2 * hmax + 1 + POT_TH - 1) / POT_TH, (ctx->kmaxmax_pot + 1 + POT_TK - 1) / POT_TK, nz);
+            k_potential<<<grid, 256, 0, st>>>(sx, sy, offsets + (size_t)z0i * nspecies, nspecies, ab, ctx->d_kmax_pot, hmax, nx,
+                                              ny, (float)(1.0 / ctx->grid.lx_A), (float)(1.0 / ctx->grid.ly_A),
+                                              d_V + (size_t)z0i * nx * ny);
+            ctx->launches++;
+        }
     }
     TACAW_CUDA(ctx, cudaGetLastError());
     return TACAW_OK;

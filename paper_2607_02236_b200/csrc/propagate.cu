@@ -219,9 +219,13 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS) k_col(ColArgs a) {
         __syncthreads();
     }
     float2 pxy[E];
+    // a column that is entirely outside the mask is never written by the row kernel: do not read it
+    // (it may hold anything, and NaN * 0 would not be 0)
+    bool col_live = true;
     if constexpr (MODE != COL_INV) {
         const float2 px = a.px[ix];
         const int km = a.kmax[ix];
+        col_live = km >= 0;
 #pragma unroll
         for (int m = 0; m < E; ++m) {
             int ky = tid + T * m;
@@ -235,7 +239,7 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS) k_col(ColArgs a) {
             float2* wc = a.waves + (size_t)w * npix + ix;
             float2 x[E];
 #pragma unroll
-            for (int m = 0; m < E; ++m) x[m] = wc[(size_t)(tid + T * m) * a.nx];
+            for (int m = 0; m < E; ++m) x[m] = col_live ? wc[(size_t)(tid + T * m) * a.nx] : make_float2(0.f, 0.f);
             if constexpr (MODE != COL_INV) {
                 fft_regs<N, E, WC, false, TWREG>(x, tw, roots_s, smA, smB, tid, c, sync);
                 if constexpr (fft_nexch<N, E>() & 1) { float2* t_ = smA; smA = smB; smB = t_; }

@@ -36,10 +36,13 @@ class Runner:
             per_frame = 8 * npix * (sum(self.nsl) + self.P)
             frames_per_block = max(1, min(wl.nframes, int(8e9 // per_frame)))
         self.fpb = int(frames_per_block)
-        self.trans = [[torch.empty((s, wl.ny, wl.nx), dtype=torch.complex64, device=self.dev) for s in self.nsl]
-                      for _ in range(self.fpb)]
+        # one [fpb][S_k][ny][nx] tensor per z-segment (tacaw_build_slices is batched over frames);
+        # trans[f][k] are views of it
+        self.trans_seg = [torch.empty((self.fpb, s, wl.ny, wl.nx), dtype=torch.complex64, device=self.dev) for s in self.nsl]
+        self.trans = [[self.trans_seg[k][f] for k in range(self.nseg)] for f in range(self.fpb)]
         self.waves = torch.empty((self.fpb * self.P, wl.ny, wl.nx), dtype=torch.complex64, device=self.dev)
-        self.species_d = [torch.from_numpy(np.ascontiguousarray(s.species, dtype=np.int32)).to(self.dev) for s in wl.segments]
+        self.species_h = [np.ascontiguousarray(s.species, dtype=np.int32) for s in wl.segments]
+        self.species_d = [torch.from_numpy(s).to(self.dev) for s in self.species_h]
         self.buf = None
 
     def alloc_buffer(self, nframes: Optional[int] = None):
@@ -52,10 +55,15 @@ class Runner:
         return [self.torch.from_numpy(seg.frames(f0, f1, self.wl.dt_fs)).to(self.dev) for seg in self.wl.segments]
 
     def build_block(self, pos_d, nf: int):
-        for i in range(nf):
-            for k, seg in enumerate(self.wl.segments):
-                self.tc.build_slices(pos_d[k][i], self.species_d[k], self.wl.a, self.wl.b, self.wl.dz, seg.nslices, 0.0,
-                                     out=self.trans[i][k])
+        for k, seg in enumerate(self.wl.segments):
+            self.tc.build_slices(pos_d[k][:nf], self.species_d[k], self.wl.a, self.wl.b, self.wl.dz, seg.nslices, 0.0,
+                                 out=self.trans_seg[k][:nf])
+
+    def build_block_host(self, pos_h, f0: int, nf: int):
+        """Same from HOST position arrays [T][Na][3] (tacaw_build_slices_host)."""
+        for k, seg in enumerate(self.wl.segments):
+            self.tc.build_slices_host(pos_h[k][f0:f0 + nf], self.species_h[k], self.wl.a, self.wl.b, self.wl.dz,
+                                      seg.nslices, 0.0, self.trans_seg[k][:nf])
 
     def propagate_block(self, nf: int, output_space: int = 1):
         nw = nf * self.P

@@ -60,11 +60,16 @@ def test_propagate_random_slices_all_grid_sizes(torch, B, oracle, n, bandlimit):
     trans, psi, wf = random_setup(n, n, n, nw, nframes, nsl)
     tc = B.Tacaw(n, n, L, L, lam, 9.2e-4, bandlimit)
     tr_d = [[dev(torch, t, torch.complex64) for t in fr] for fr in trans]
+    probes = dev(torch, psi, torch.complex64)
     for space in (0, 1):
         ref = oracle.propagate(L, L, lam, bandlimit, psi, wf, trans, dz, space)
-        w = dev(torch, psi, torch.complex64)
-        tc.propagate(w, wf, tr_d, dz, space)
+        # output buffer pre-filled with NaN: nothing of its previous content may leak into the result
+        w = torch.full((nw, n, n), float("nan"), dtype=torch.complex64, device="cuda")
+        tc.propagate(w, wf, tr_d, dz, space, probes=probes, wave_probe=np.arange(nw, dtype=np.int32))
         got = w.cpu().numpy()
+        w2 = dev(torch, psi, torch.complex64)
+        tc.propagate(w2, wf, tr_d, dz, space)                    # in-place variant (entrance waves in d_waves)
+        assert torch.equal(w2, w)
         for i in range(nw):
             assert rel_l2(got[i], ref[i]) <= 2e-5, (n, space, i)
         if space == 1 and bandlimit:
@@ -166,6 +171,25 @@ def test_build_slices_vs_oracle(torch, B, oracle, case):
     phase_scale = max(1.0, wl.sigma * np.abs(ref["v"]).max())
     for n in range(seg.nslices):
         assert rel_l2(got[n], ref["trans"][n]) <= 2e-6 * phase_scale, (case, n)
+    tc.close()
+
+
+def test_build_slices_batched_over_frames(torch, B, oracle):
+    """One call for several frames == one call per frame == oracle."""
+    wl = W.make_workload(1)
+    seg = wl.segments[0]
+    pos = seg.frames(0, 5, wl.dt_fs)
+    tc = B.Tacaw(wl.nx, wl.ny, wl.lx, wl.ly, wl.lam, wl.sigma, 1)
+    out = torch.full((5, seg.nslices, wl.ny, wl.nx), float("nan"), dtype=torch.complex64, device="cuda")
+    tb, ncl = tc.build_slices(dev(torch, pos), dev(torch, seg.species), wl.a, wl.b, wl.dz, seg.nslices, 0.0, out=out,
+                              want_clamped=True)
+    assert ncl == 0
+    for f in range(5):
+        t1, _ = tc.build_slices(dev(torch, pos[f]), dev(torch, seg.species), wl.a, wl.b, wl.dz, seg.nslices, 0.0)
+        assert torch.equal(tb[f], t1)
+        ref = oracle.build_slices(wl.nx, wl.ny, wl.lx, wl.ly, pos[f], seg.species, wl.a, wl.b, wl.dz, seg.nslices, 0.0,
+                                  wl.sigma, 1, 1)
+        assert rel_l2(tb[f].cpu().numpy(), ref["trans"]) <= 1e-5
     tc.close()
 
 
