@@ -171,6 +171,10 @@ int tacaw_create(tacaw_ctx** out, const tacaw_grid* grid, const tacaw_beam* beam
          cudaMemcpy(ctx->d_roots_y, ry.data(), sizeof(float2) * ny, cudaMemcpyHostToDevice) == cudaSuccess &&
          cudaMemcpy(ctx->d_kmax, ctx->kmax.data(), sizeof(int) * nx, cudaMemcpyHostToDevice) == cudaSuccess &&
          cudaMemcpy(ctx->d_kmax_pot, ctx->kmax_pot.data(), sizeof(int) * nx, cudaMemcpyHostToDevice) == cudaSuccess;
+    ok = ok && cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming) == cudaSuccess;
+    for (int i = 0; i < tacaw_ctx::MAX_AUX; ++i)
+        ok = ok && cudaStreamCreateWithFlags(&ctx->aux[i], cudaStreamNonBlocking) == cudaSuccess &&
+             cudaEventCreateWithFlags(&ctx->ev_join[i], cudaEventDisableTiming) == cudaSuccess;
     if (!ok) {
         (void)cudaGetLastError();
         tacaw_destroy(ctx);
@@ -187,6 +191,11 @@ int tacaw_destroy(tacaw_ctx* ctx) {
     cudaFree(ctx->d_px); cudaFree(ctx->d_py); cudaFree(ctx->d_meta); cudaFree(ctx->d_sort); cudaFree(ctx->d_stage);
     cudaFree(ctx->d_spec_tab);
     if (ctx->h_arena) cudaFreeHost(ctx->h_arena);
+    for (int i = 0; i < tacaw_ctx::MAX_AUX; ++i) {
+        if (ctx->aux[i]) cudaStreamDestroy(ctx->aux[i]);
+        if (ctx->ev_join[i]) cudaEventDestroy(ctx->ev_join[i]);
+    }
+    if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
     (void)cudaGetLastError();
     delete ctx;
     return TACAW_OK;
@@ -361,7 +370,8 @@ int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, const i
 
     // depth-first over groups of waves small enough to stay L2-resident between the two kernels of
     // a slice step: all slices for group 0, then group 1, ...
-    size_t budget = ctx->l2_bytes ? ctx->l2_bytes / 2 : (size_t)48 << 20;
+    // a few groups are in flight at once (one per stream)
+    size_t budget = ctx->l2_bytes ? ctx->l2_bytes / 2 : (size_t)64 << 20;
     if (const char* e = getenv("TACAW_L2_GROUP_MB")) {
         double mb = atof(e);
         if (mb > 0) budget = (size_t)(mb * 1048576.0);
@@ -369,8 +379,21 @@ int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, const i
     int gmax = (int)(budget / (npix * sizeof(float2)));
     if (gmax < 1) gmax = 1;
     const int ngroups = (nwaves + gmax - 1) / gmax;
+    static const int max_streams = [] {
+        const char* e = getenv("TACAW_STREAMS");
+        int v = e ? atoi(e) : 2;
+        return v < 1 ? 1 : (v > 1 + tacaw_ctx::MAX_AUX ? 1 + tacaw_ctx::MAX_AUX : v);
+    }();
+    const int nstreams = ngroups < max_streams ? ngroups : max_streams;
+    const bool fork = nstreams >= 2;
+    cudaStream_t user_st = st;
+    if (fork) {
+        TACAW_CUDA(ctx, cudaEventRecord(ctx->ev_fork, user_st));
+        for (int i = 0; i + 1 < nstreams; ++i) TACAW_CUDA(ctx, cudaStreamWaitEvent(ctx->aux[i], ctx->ev_fork, 0));
+    }
     int w0 = 0;
     for (int gi = 0; gi < ngroups; ++gi) {
+        st = (gi % nstreams) ? ctx->aux[gi % nstreams - 1] : user_st;
         // balanced groups; a boundary moves to the nearest frame change within a quarter group
         int w1 = (int)(((long long)(gi + 1) * nwaves) / ngroups);
         if (gi + 1 < ngroups) {
@@ -413,6 +436,12 @@ int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, const i
             if (rc) return rc;
         }
         w0 = w1;
+    }
+    if (fork) {
+        for (int i = 0; i + 1 < nstreams; ++i) {
+            TACAW_CUDA(ctx, cudaEventRecord(ctx->ev_join[i], ctx->aux[i]));
+            TACAW_CUDA(ctx, cudaStreamWaitEvent(user_st, ctx->ev_join[i], 0));
+        }
     }
     return TACAW_OK;
 }

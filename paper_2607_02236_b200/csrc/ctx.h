@@ -43,6 +43,12 @@ struct tacaw_ctx {
     char* h_arena = nullptr;
     size_t arena_bytes = 0, arena_off = 0;
 
+    // second stream: tacaw_propagate runs alternate wave groups on it so one group's kernel tails
+    // overlap the other group's kernels (fork/join with events around the call)
+    static constexpr int MAX_AUX = 3;
+    cudaStream_t aux[MAX_AUX] = {nullptr, nullptr, nullptr};
+    cudaEvent_t ev_fork = nullptr, ev_join[MAX_AUX] = {nullptr, nullptr, nullptr};
+
     std::string err;
     int64_t launches = 0;
 };

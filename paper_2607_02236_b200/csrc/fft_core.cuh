@@ -9,15 +9,19 @@
 // jb = tid + b*T, outputs to index (jb/Ns)*Ns*R + k + t*Ns.
 // WC transforms that are interleaved in memory (a [N][WC] column tile) are handled as one
 // transform over vectors: shared index = a*WC + c.
-// Exchanges use 64-bit shared accesses; the XOR swizzle below makes every half-warp wavefront
-// bank-conflict free for all (N, E, WC) used here (checked by enumeration).
+// Exchanges use 64-bit shared accesses into a padded buffer, index P(A) = A + ((A >> 4) << u): the
+// pad makes every half-warp wavefront bank-conflict free for all (N, E, WC) used here AND keeps the
+// per-output / per-element offsets additive compile-time constants (both checked by enumeration,
+// see DESIGN.md), so an exchange costs one base address computation plus immediate offsets.
+// Butterflies use the sm_100 packed fp32x2 instructions (FADD2 / FFMA2): a complex add is one
+// instruction and the +-i rotations ride on FADD2's operand swizzle (LO_HI.NP) for free.
 #pragma once
 #include <cuda_runtime.h>
 
 namespace tacaw {
 
-__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return __fadd2_rn(a, make_float2(-b.x, -b.y)); }
 __device__ __forceinline__ float2 cmul(float2 a, float2 w) {
     return make_float2(fmaf(a.x, w.x, -a.y * w.y), fmaf(a.x, w.y, a.y * w.x));
 }
@@ -34,80 +38,101 @@ template <bool INV>
 __device__ __forceinline__ float2 mul_mi(float2 a) {
     return INV ? make_float2(-a.y, a.x) : make_float2(a.y, -a.x);
 }
+// scalar variants for values that are stored right away: ptxas puts a MOV pair between a packed
+// FADD2/FFMA2 result and an STS/STG that consumes it, so the last butterfly stage before a store
+// is cheaper in scalar fp32 (2 FADD) than packed (FADD2 + 2 MOV)
+template <bool S>
+__device__ __forceinline__ float2 caddS(float2 a, float2 b) {
+    return S ? make_float2(a.x + b.x, a.y + b.y) : __fadd2_rn(a, b);
+}
+template <bool S>
+__device__ __forceinline__ float2 csubS(float2 a, float2 b) {
+    return S ? make_float2(a.x - b.x, a.y - b.y) : __fadd2_rn(a, make_float2(-b.x, -b.y));
+}
+template <bool S>
+__device__ __forceinline__ float2 axpyS(float s, float2 t, float2 e) {
+    return S ? make_float2(fmaf(s, t.x, e.x), fmaf(s, t.y, e.y)) : __ffma2_rn(t, make_float2(s, s), e);
+}
+// a + (-+i) b  and  a - (-+i) b  (one FADD2 each: the rotation is an operand swizzle)
+template <bool INV, bool S = false>
+__device__ __forceinline__ float2 add_mi(float2 a, float2 b) { return caddS<S>(a, mul_mi<INV>(b)); }
+template <bool INV, bool S = false>
+__device__ __forceinline__ float2 sub_mi(float2 a, float2 b) { return caddS<S>(a, mul_mi<!INV>(b)); }
+// e + s*t (s real)
+__device__ __forceinline__ float2 axpy(float s, float2 t, float2 e) { return __ffma2_rn(t, make_float2(s, s), e); }
 
 constexpr __host__ __device__ int ilog2c(int v) { return v <= 1 ? 0 : 1 + ilog2c(v >> 1); }
 
 // ---------------------------------------------------------------------------------------------
 // In-register DFTs of size R, natural order in and out.  Forward = exp(-2 pi i st/R).
-template <int R, bool INV>
+// SOUT: the outputs are stored right away (scalar last stage, see caddS).
+template <int R, bool INV, bool SOUT = false>
 struct Dft;
 
-template <bool INV>
-struct Dft<1, INV> {
+template <bool INV, bool SOUT>
+struct Dft<1, INV, SOUT> {
     static __device__ __forceinline__ void run(float2 (&)[1]) {}
 };
 
-template <bool INV>
-struct Dft<2, INV> {
+template <bool INV, bool SOUT>
+struct Dft<2, INV, SOUT> {
     static __device__ __forceinline__ void run(float2 (&v)[2]) {
         float2 a = v[0], b = v[1];
-        v[0] = cadd(a, b);
-        v[1] = csub(a, b);
+        v[0] = caddS<SOUT>(a, b);
+        v[1] = csubS<SOUT>(a, b);
     }
 };
 
-template <bool INV>
-struct Dft<4, INV> {
+template <bool INV, bool SOUT>
+struct Dft<4, INV, SOUT> {
     static __device__ __forceinline__ void run(float2 (&v)[4]) {
         float2 t0 = cadd(v[0], v[2]), t1 = csub(v[0], v[2]);
-        float2 t2 = cadd(v[1], v[3]), t3 = mul_mi<INV>(csub(v[1], v[3]));
-        v[0] = cadd(t0, t2);
-        v[1] = cadd(t1, t3);
-        v[2] = csub(t0, t2);
-        v[3] = csub(t1, t3);
+        float2 t2 = cadd(v[1], v[3]), t3 = csub(v[1], v[3]);
+        v[0] = caddS<SOUT>(t0, t2);
+        v[2] = csubS<SOUT>(t0, t2);
+        v[1] = add_mi<INV, SOUT>(t1, t3);
+        v[3] = sub_mi<INV, SOUT>(t1, t3);
     }
 };
 
-template <bool INV>
-struct Dft<8, INV> {
+template <bool INV, bool SOUT>
+struct Dft<8, INV, SOUT> {
     static __device__ __forceinline__ void run(float2 (&v)[8]) {
         float2 e[4] = {v[0], v[2], v[4], v[6]};
         float2 o[4] = {v[1], v[3], v[5], v[7]};
-        Dft<4, INV>::run(e);
-        Dft<4, INV>::run(o);
+        Dft<4, INV, false>::run(e);
+        Dft<4, INV, false>::run(o);
         const float c = 0.70710678118654752440f;
-        // o1 *= w8, o2 *= w8^2 = -+i, o3 *= w8^3
-        float2 o1 = INV ? make_float2(c * (o[1].x - o[1].y), c * (o[1].x + o[1].y))
-                        : make_float2(c * (o[1].x + o[1].y), c * (o[1].y - o[1].x));
-        float2 o2 = mul_mi<INV>(o[2]);
-        float2 o3 = INV ? make_float2(-c * (o[3].x + o[3].y), c * (o[3].x - o[3].y))
-                        : make_float2(c * (o[3].y - o[3].x), -c * (o[3].x + o[3].y));
-        v[0] = cadd(e[0], o[0]); v[4] = csub(e[0], o[0]);
-        v[1] = cadd(e[1], o1);   v[5] = csub(e[1], o1);
-        v[2] = cadd(e[2], o2);   v[6] = csub(e[2], o2);
-        v[3] = cadd(e[3], o3);   v[7] = csub(e[3], o3);
+        // o1 w8 = c (o1 + (-+i) o1);   o3 w8^3 = -c (o3 - (-+i) o3)
+        float2 t1 = add_mi<INV>(o[1], o[1]);
+        float2 t3 = sub_mi<INV>(o[3], o[3]);
+        v[0] = caddS<SOUT>(e[0], o[0]);        v[4] = csubS<SOUT>(e[0], o[0]);
+        v[1] = axpyS<SOUT>(c, t1, e[1]);       v[5] = axpyS<SOUT>(-c, t1, e[1]);
+        v[2] = add_mi<INV, SOUT>(e[2], o[2]);  v[6] = sub_mi<INV, SOUT>(e[2], o[2]);
+        v[3] = axpyS<SOUT>(-c, t3, e[3]);      v[7] = axpyS<SOUT>(c, t3, e[3]);
     }
 };
 
-template <bool INV>
-struct Dft<16, INV> {
+template <bool INV, bool SOUT>
+struct Dft<16, INV, SOUT> {
     static __device__ __forceinline__ void run(float2 (&v)[16]) {
         float2 e[8], o[8];
 #pragma unroll
         for (int i = 0; i < 8; ++i) { e[i] = v[2 * i]; o[i] = v[2 * i + 1]; }
-        Dft<8, INV>::run(e);
-        Dft<8, INV>::run(o);
+        Dft<8, INV, false>::run(e);
+        Dft<8, INV, false>::run(o);
         // w16^k = (cos(k pi/8), -sin(k pi/8)) forward
         const float c1 = 0.92387953251128675613f, s1 = 0.38268343236508977173f;
         const float c2 = 0.70710678118654752440f;
-        const float2 w[8] = {make_float2(1.f, 0.f),  make_float2(c1, -s1),  make_float2(c2, -c2), make_float2(s1, -c1),
-                             make_float2(0.f, -1.f), make_float2(-s1, -c1), make_float2(-c2, -c2), make_float2(-c1, -s1)};
-#pragma unroll
-        for (int k = 0; k < 8; ++k) {
-            float2 t = (k == 0) ? o[0] : (k == 4 ? mul_mi<INV>(o[4]) : cmul_dir<INV>(o[k], w[k]));
-            v[k] = cadd(e[k], t);
-            v[k + 8] = csub(e[k], t);
-        }
+        constexpr bool S = SOUT;
+        v[0] = caddS<S>(e[0], o[0]);  v[8] = csubS<S>(e[0], o[0]);
+        {   float2 t = cmul_dir<INV>(o[1], make_float2(c1, -s1));  v[1] = caddS<S>(e[1], t);  v[9] = csubS<S>(e[1], t); }
+        {   float2 t = add_mi<INV>(o[2], o[2]);  v[2] = axpyS<S>(c2, t, e[2]);  v[10] = axpyS<S>(-c2, t, e[2]); }
+        {   float2 t = cmul_dir<INV>(o[3], make_float2(s1, -c1));  v[3] = caddS<S>(e[3], t);  v[11] = csubS<S>(e[3], t); }
+        v[4] = add_mi<INV, S>(e[4], o[4]);  v[12] = sub_mi<INV, S>(e[4], o[4]);
+        {   float2 t = cmul_dir<INV>(o[5], make_float2(-s1, -c1)); v[5] = caddS<S>(e[5], t);  v[13] = csubS<S>(e[5], t); }
+        {   float2 t = sub_mi<INV>(o[6], o[6]);  v[6] = axpyS<S>(-c2, t, e[6]);  v[14] = axpyS<S>(c2, t, e[6]); }
+        {   float2 t = cmul_dir<INV>(o[7], make_float2(-c1, -s1)); v[7] = caddS<S>(e[7], t);  v[15] = csubS<S>(e[7], t); }
     }
 };
 
@@ -124,12 +149,15 @@ struct FftPlan {
     static constexpr int NEXCH = (N > E) ? ((N / E > E) ? 2 + (N / E / E > E ? 1 : 0) : 1) : 0;  // informational
 };
 
-// XOR swizzle of a shared index (float2 units); nsw = Ns*WC of the pass that writes.
-template <int NSW, int R>
-__device__ __forceinline__ int swz(int a) {
-    if (NSW >= 16) return a;
-    return a ^ (((a >> ilog2c(NSW * R)) << ilog2c(NSW)) & 15);
+// Padded shared index P(A) = A + ((A >> 4) << u) for the exchange written by the pass (NS, R) of
+// a transform over WC interleaved columns; u < 0 means no pad.  Rule found by exhaustive search:
+// conflict-free writes and reads per half-warp, offsets additive (see header comment).
+constexpr __host__ __device__ int pad_u(int wc, int ns, int r) {
+    return (ns * wc >= 16) ? -1 : (wc == 1 ? (ns == 1 ? 0 : 1) : (r == 8 ? 1 : 0));
 }
+constexpr __host__ __device__ int pad_idx(int a, int u) { return u < 0 ? a : a + ((a >> 4) << u); }
+// float2 elements an exchange buffer needs for a transform of n points over wc columns
+constexpr __host__ __device__ int exch_elems(int n, int wc) { return n * wc + (n * wc) / 8; }
 
 // Fill this thread's twiddle registers from the table roots[j] = exp(-2 pi i j/N) (fp64-accurate).
 template <int N, int E, int NS, int OFF>
@@ -155,7 +183,7 @@ struct TwInit {
 // The passes.  x: registers; smA/smB: ping-pong exchange buffers of N*WC float2 each;
 // tid in [0,T), c in [0,WC).  TWREG: twiddles from registers `tw`; else from the shared table
 // `roots` (N float2).  Sync: functor that synchronises the T*WC threads of this transform group.
-template <int N, int E, int WC, bool INV, bool TWREG, int NS, int OFF>
+template <int N, int E, int WC, bool INV, bool TWREG, bool STORE_AFTER, int NS, int OFF>
 struct FftPass {
     using P = FftPlan<N, E>;
     static constexpr int R = P::radix(NS);
@@ -164,9 +192,17 @@ struct FftPass {
     static constexpr bool LAST = (NS * R == N);
     static constexpr int NTWH = (NS > 1) ? (R - 1) * NB : 0;
 
+    static constexpr int U = pad_u(WC, NS, R);
+    // compile-time offsets relative to the padded base (thread-independent by construction)
+    static constexpr __host__ __device__ int woff(int b, int t) {
+        const int b0 = b * T, k0 = b0 & (NS - 1), base0 = ((b0 - k0) * R + k0) * WC;
+        return pad_idx(base0 + t * NS * WC, U) - pad_idx(base0, U);
+    }
+    static constexpr __host__ __device__ int roff(int m) { return pad_idx(T * m * WC, U); }
+
     template <class Sync>
     static __device__ __forceinline__ void run(float2 (&x)[E], const float2 (&tw)[P::NTW], const float2* roots,
-                                               float2* smA, float2* smB, int tid, int c, Sync sync) {
+                                               float2* smA, float2* smB, int tid, int c, Sync& sync) {
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
             float2 v[R];
@@ -183,29 +219,31 @@ struct FftPass {
                     v[t] = cmul_dir<INV>(v[t], w);
                 }
             }
-            Dft<R, INV>::run(v);
+            Dft<R, INV, (!LAST) || STORE_AFTER>::run(v);
             if constexpr (LAST) {
 #pragma unroll
                 for (int t = 0; t < R; ++t) x[b + t * NB] = v[t];
             } else {
-                const int base = (jb - k) * R + k;
+                float2* wp = smA + pad_idx(((jb - k) * R + k) * WC + c, U);
 #pragma unroll
-                for (int t = 0; t < R; ++t) smA[swz<NS * WC, R>((base + t * NS) * WC + c)] = v[t];
+                for (int t = 0; t < R; ++t) wp[woff(b, t)] = v[t];
             }
         }
         if constexpr (!LAST) {
             sync();
+            const float2* rp = smA + pad_idx(tid * WC + c, U);
 #pragma unroll
-            for (int m = 0; m < E; ++m) x[m] = smA[swz<NS * WC, R>((tid + T * m) * WC + c)];
-            FftPass<N, E, WC, INV, TWREG, NS * R, OFF + NTWH>::run(x, tw, roots, smB, smA, tid, c, sync);
+            for (int m = 0; m < E; ++m) x[m] = rp[roff(m)];
+            FftPass<N, E, WC, INV, TWREG, STORE_AFTER, NS * R, OFF + NTWH>::run(x, tw, roots, smB, smA, tid, c, sync);
         }
     }
 };
 
-template <int N, int E, int WC, bool INV, bool TWREG, class Sync>
+// STORE_AFTER: the transform's outputs go straight to a global store (no arithmetic in between).
+template <int N, int E, int WC, bool INV, bool TWREG, bool STORE_AFTER = false, class Sync>
 __device__ __forceinline__ void fft_regs(float2 (&x)[E], const float2 (&tw)[FftPlan<N, E>::NTW], const float2* roots,
-                                         float2* smA, float2* smB, int tid, int c, Sync sync) {
-    FftPass<N, E, WC, INV, TWREG, 1, 0>::run(x, tw, roots, smA, smB, tid, c, sync);
+                                         float2* smA, float2* smB, int tid, int c, Sync& sync) {
+    FftPass<N, E, WC, INV, TWREG, STORE_AFTER, 1, 0>::run(x, tw, roots, smA, smB, tid, c, sync);
 }
 
 // number of exchanges of a plan (so callers know which ping-pong buffer the next transform may use)
@@ -230,5 +268,13 @@ struct SyncNamed {
     int id, count;
     __device__ __forceinline__ void operator()() const { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory"); }
 };
+
+// 16-byte asynchronous global -> shared copy (LDGSTS), bypassing L1 and registers.
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
+    unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
 }  // namespace tacaw

@@ -10,10 +10,23 @@
 // ROW_FIRST starts from the r-space entrance wave; ROW_LAST returns to r space; COL_LASTQ stops
 // after the propagator multiply and stores the q-space exit wave Psi_S.  ROW_TRANS / COL_INV are
 // the same transforms used by tacaw_build_slices and tacaw_make_probes.
+#include <cstdlib>
+
 #include "ctx.h"
 #include "fft_core.cuh"
 
 namespace tacaw {
+
+// CTAs per launch aimed for (x SM count): a CTA loops over ceil(nwaves/chunks) waves, prefetching the
+// next one while it transforms the current one.  TACAW_CTAS_PER_SM overrides (tuning only).
+static int cta_target(const tacaw_ctx* ctx) {
+    static int per_sm = [] {
+        const char* e = getenv("TACAW_CTAS_PER_SM");
+        int v = e ? atoi(e) : 0;
+        return v > 0 ? v : 4;
+    }();
+    return ctx->num_sms * per_sm;
+}
 
 // ------------------------------------------------------------------------------------------
 template <int N>
@@ -24,71 +37,125 @@ struct RowCfg {
     static constexpr bool TWREG = (E == 8);
 };
 
+// Barrier functor that, the first time it fires after being armed, also issues the asynchronous
+// prefetch of the next wave (every thread of the group has read the staging buffers by then).
+template <class Base, class Issue>
+struct SyncPrefetch {
+    Base base;
+    Issue issue;
+    bool armed;
+    __device__ __forceinline__ void operator()() {
+        base();
+        if (armed) {
+            armed = false;
+            issue();
+        }
+    }
+};
+
 template <int N, int MODE>
 __global__ void __launch_bounds__(RowCfg<N>::THREADS) k_row(RowArgs a) {
     using C = RowCfg<N>;
     constexpr int E = C::E, T = C::T;
     constexpr bool TWREG = C::TWREG;
+    constexpr bool HAS_T = (MODE == ROW_FIRST || MODE == ROW_MID);
+    constexpr int XE = exch_elems(N, 1);
+    constexpr int PER_G = 2 * XE + (HAS_T ? 2 : 1) * N;     // exchange A, exchange B, wave stage, t stage
     using P = FftPlan<N, E>;
-    extern __shared__ float2 smem[];
+    extern __shared__ __align__(16) float2 smem[];
     const int lt = threadIdx.x;
     const int g = lt / T, tid = lt % T;
     const int G = blockDim.x / T;
     const int row = blockIdx.x * G + g;
-    float2* smA = smem + (size_t)g * 2 * N;
-    float2* smB = smA + N;
+    float2* smA = smem + (size_t)g * PER_G;
+    float2* smB = smA + XE;
+    float2* sW = smA + 2 * XE;
+    float2* sT = sW + N;
     const float2* roots_s = nullptr;
     float2 tw[P::NTW];
     if constexpr (TWREG) {
         TwInit<N, E, 1, 0>::run(tw, a.roots, tid);
     } else {
-        float2* rs = smem + (size_t)G * 2 * N;
+        float2* rs = smem + (size_t)G * PER_G;
         for (int i = lt; i < N; i += blockDim.x) rs[i] = a.roots[i];
         roots_s = rs;
         __syncthreads();
     }
-    auto body = [&](auto sync) {
-        const int w0 = blockIdx.y * a.wpc;
-        const int w1 = min(w0 + a.wpc, a.nwaves);
-        const size_t npix = (size_t)a.ny * N;
-        int cur_frame = -1;
-        float2 tr[E];
-        bool inb[E];
+    const int w0 = blockIdx.y * a.wpc;
+    const int w1 = min(w0 + a.wpc, a.nwaves);
+    const size_t npix = (size_t)a.ny * N;
+    const size_t rowoff = (size_t)row * N;
+    bool inb[E];
 #pragma unroll
-        for (int m = 0; m < E; ++m) {
-            int ix = tid + T * m;
-            inb[m] = (ix <= a.hmax) || (ix >= N - a.hmax);
+    for (int m = 0; m < E; ++m) {
+        int ix = tid + T * m;
+        inb[m] = (MODE == ROW_FIRST) || (ix <= a.hmax) || (ix >= N - a.hmax);
+    }
+    // asynchronous staging (LDGSTS, 16 B chunks): wave row -> sW (in-band chunks only), t row -> sT
+    auto issue = [&](int w, bool with_t) {
+        const float2* src;
+        if constexpr (MODE == ROW_FIRST) src = a.probes ? a.probes + (size_t)a.wave_probe[w] * npix + rowoff
+                                                        : a.waves + (size_t)w * npix + rowoff;
+        else src = a.waves + (size_t)w * npix + rowoff;
+#pragma unroll
+        for (int j = 0; j < E / 2; ++j) {
+            const int ix0 = 2 * (tid + T * j);
+            const bool p = (MODE == ROW_FIRST) || (ix0 <= a.hmax) || (ix0 + 1 >= N - a.hmax);
+            if (p) cp_async16(sW + ix0, src + ix0);
         }
-        for (int w = w0; w < w1; ++w) {
-            float2 x[E];
-            float2* wrow = a.waves + (size_t)w * npix + (size_t)row * N;
-            if constexpr (MODE == ROW_FIRST || MODE == ROW_MID) {
-                int f = a.wave_frame[w];
-                if (f != cur_frame) {
-                    const float2* tp = a.trans[(size_t)f * a.nseg + a.seg] + (size_t)a.slice * npix + (size_t)row * N;
+        if constexpr (HAS_T) {
+            if (with_t) {
+                const float2* tp = a.trans[(size_t)a.wave_frame[w] * a.nseg + a.seg] + (size_t)a.slice * npix + rowoff;
 #pragma unroll
-                    for (int m = 0; m < E; ++m) tr[m] = __ldg(tp + tid + T * m);
+                for (int j = 0; j < E / 2; ++j) {
+                    const int ix0 = 2 * (tid + T * j);
+                    cp_async16(sT + ix0, tp + ix0);
+                }
+            }
+        }
+        cp_async_commit();
+    };
+    auto body = [&](auto base_sync) {
+        int cur_frame = -1;
+        int next_w = w0;
+        bool next_t = true;
+        auto pf = [&]() { issue(next_w, next_t); };
+        SyncPrefetch<decltype(base_sync), decltype(pf)> sync{base_sync, pf, false};
+        if (w0 < w1) issue(w0, true);
+        float2 tr[E];
+        for (int w = w0; w < w1; ++w) {
+            cp_async_wait_all();
+            base_sync();
+            float2 x[E];
+#pragma unroll
+            for (int m = 0; m < E; ++m) x[m] = inb[m] ? sW[tid + T * m] : make_float2(0.f, 0.f);
+            if constexpr (HAS_T) {
+                const int f = a.wave_frame[w];
+                if (f != cur_frame) {
+#pragma unroll
+                    for (int m = 0; m < E; ++m) tr[m] = sT[tid + T * m];
                     cur_frame = f;
                 }
             }
-            if constexpr (MODE == ROW_FIRST) {
-                const float2* src = a.probes ? a.probes + (size_t)a.wave_probe[w] * npix + (size_t)row * N : wrow;
-#pragma unroll
-                for (int m = 0; m < E; ++m) x[m] = src[tid + T * m];
-            } else {
-#pragma unroll
-                for (int m = 0; m < E; ++m) x[m] = inb[m] ? wrow[tid + T * m] : make_float2(0.f, 0.f);
-                fft_regs<N, E, 1, true, TWREG>(x, tw, roots_s, smA, smB, tid, 0, sync);
+            if (w + 1 < w1) {
+                next_w = w + 1;
+                if constexpr (HAS_T) next_t = a.wave_frame[w + 1] != cur_frame;
+                sync.armed = true;
+            }
+            float2* wrow = a.waves + (size_t)w * npix + rowoff;
+            if constexpr (MODE != ROW_FIRST) {
+                fft_regs<N, E, 1, true, TWREG, MODE == ROW_LAST>(x, tw, roots_s, smA, smB, tid, 0, sync);
                 if constexpr (fft_nexch<N, E>() & 1) { float2* t_ = smA; smA = smB; smB = t_; }
             }
-            if constexpr (MODE == ROW_FIRST || MODE == ROW_MID) {
+            if constexpr (HAS_T) {
 #pragma unroll
                 for (int m = 0; m < E; ++m) x[m] = cmul(x[m], tr[m]);
-                fft_regs<N, E, 1, false, TWREG>(x, tw, roots_s, smA, smB, tid, 0, sync);
+                fft_regs<N, E, 1, false, TWREG, true>(x, tw, roots_s, smA, smB, tid, 0, sync);
                 if constexpr (fft_nexch<N, E>() & 1) { float2* t_ = smA; smA = smB; smB = t_; }
 #pragma unroll
                 for (int m = 0; m < E; ++m)
-                    if (inb[m]) wrow[tid + T * m] = x[m];
+                    if (MODE == ROW_FIRST ? ((tid + T * m <= a.hmax) || (tid + T * m >= N - a.hmax)) : inb[m])
+                        wrow[tid + T * m] = x[m];
             } else if constexpr (MODE == ROW_LAST) {
 #pragma unroll
                 for (int m = 0; m < E; ++m) wrow[tid + T * m] = x[m];
@@ -119,13 +186,14 @@ static int launch_row_n(tacaw_ctx* ctx, const RowArgs& a0, cudaStream_t st) {
     if (G > a.ny) G = a.ny;
     int threads = G * C::T;
     int nrb = a.ny / G;
-    int target = ctx->num_sms * 8;
+    int target = cta_target(ctx);
     int nchunks = target / nrb;
     if (nchunks < 1) nchunks = 1;
     if (nchunks > a.nwaves) nchunks = a.nwaves;
     a.wpc = (a.nwaves + nchunks - 1) / nchunks;
     nchunks = (a.nwaves + a.wpc - 1) / a.wpc;
-    size_t smem = (size_t)G * 2 * N * sizeof(float2) + (C::TWREG ? 0 : (size_t)N * sizeof(float2));
+    const int per_g = 2 * exch_elems(N, 1) + ((MODE == ROW_FIRST || MODE == ROW_MID) ? 2 : 1) * N;
+    size_t smem = (size_t)G * per_g * sizeof(float2) + (C::TWREG ? 0 : (size_t)N * sizeof(float2));
     auto kern = k_row<N, MODE>;
     if (smem > 48 * 1024) TACAW_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     kern<<<dim3(nrb, nchunks), threads, smem, st>>>(a);
@@ -176,11 +244,12 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS) k_col(ColArgs a) {
     constexpr int E = C::E, T = C::T, WC = C::WC;
     constexpr bool TWREG = C::TWREG;
     using P = FftPlan<N, E>;
-    extern __shared__ float2 smem[];
+    extern __shared__ __align__(16) float2 smem[];
     const int lt = threadIdx.x;
     const int c = lt % WC, tid = lt / WC;
+    constexpr int XE = exch_elems(N, WC);
     float2* smA = smem;
-    float2* smB = smem + (size_t)N * WC;
+    float2* smB = smem + XE;
     const float2* roots_s = nullptr;
     // column group of this CTA
     const int NG = a.nx / WC;
@@ -209,17 +278,18 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS) k_col(ColArgs a) {
         return;
     }
 
+    float2* sW = smem + 2 * XE;                  // staging tile [N][WC]
     float2 tw[P::NTW];
     if constexpr (TWREG) {
         TwInit<N, E, 1, 0>::run(tw, a.roots, tid);
     } else {
-        float2* rs = smem + (size_t)2 * N * WC;
+        float2* rs = smem + 2 * XE + N * WC;
         for (int i = lt; i < N; i += blockDim.x) rs[i] = a.roots[i];
         roots_s = rs;
         __syncthreads();
     }
     float2 pxy[E];
-    // a column that is entirely outside the mask is never written by the row kernel: do not read it
+    // a column that is entirely outside the mask is never written by the row kernel: do not use it
     // (it may hold anything, and NaN * 0 would not be 0)
     bool col_live = true;
     if constexpr (MODE != COL_INV) {
@@ -234,12 +304,33 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS) k_col(ColArgs a) {
             pxy[m] = (k <= km) ? make_float2(p.x * a.pscale, p.y * a.pscale) : make_float2(0.f, 0.f);
         }
     }
-    auto body = [&](auto sync) {
+    // asynchronous staging of the [N][WC] tile of wave w: 16 B chunks, E/2 per thread
+    auto issue = [&](int w) {
+        const float2* src = a.waves + (size_t)w * npix + (size_t)grp * WC;
+#pragma unroll
+        for (int j = 0; j < E / 2; ++j) {
+            const int id = lt + C::THREADS * j;
+            const int r = id / (WC / 2), part = id % (WC / 2);
+            cp_async16(sW + r * WC + 2 * part, src + (size_t)r * a.nx + 2 * part);
+        }
+        cp_async_commit();
+    };
+    auto body = [&](auto base_sync) {
+        int next_w = w0;
+        auto pf = [&]() { issue(next_w); };
+        SyncPrefetch<decltype(base_sync), decltype(pf)> sync{base_sync, pf, false};
+        if (w0 < w1) issue(w0);
         for (int w = w0; w < w1; ++w) {
+            cp_async_wait_all();
+            base_sync();
             float2* wc = a.waves + (size_t)w * npix + ix;
             float2 x[E];
 #pragma unroll
-            for (int m = 0; m < E; ++m) x[m] = col_live ? wc[(size_t)(tid + T * m) * a.nx] : make_float2(0.f, 0.f);
+            for (int m = 0; m < E; ++m) x[m] = col_live ? sW[(tid + T * m) * WC + c] : make_float2(0.f, 0.f);
+            if (w + 1 < w1) {
+                next_w = w + 1;
+                sync.armed = true;
+            }
             if constexpr (MODE != COL_INV) {
                 fft_regs<N, E, WC, false, TWREG>(x, tw, roots_s, smA, smB, tid, c, sync);
                 if constexpr (fft_nexch<N, E>() & 1) { float2* t_ = smA; smA = smB; smB = t_; }
@@ -247,7 +338,7 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS) k_col(ColArgs a) {
                 for (int m = 0; m < E; ++m) x[m] = cmul(x[m], pxy[m]);
             }
             if constexpr (MODE != COL_LASTQ) {
-                fft_regs<N, E, WC, true, TWREG>(x, tw, roots_s, smA, smB, tid, c, sync);
+                fft_regs<N, E, WC, true, TWREG, true>(x, tw, roots_s, smA, smB, tid, c, sync);
                 if constexpr (fft_nexch<N, E>() & 1) { float2* t_ = smA; smA = smB; smB = t_; }
             }
 #pragma unroll
@@ -268,13 +359,13 @@ static int launch_col_n(tacaw_ctx* ctx, const ColArgs& a0, cudaStream_t st) {
         int nlo = a.hmax / C::WC + 1, nhi = (a.hmax + C::WC - 1) / C::WC;
         if (nlo + nhi < NG) ngroups = nlo + nhi;
     }
-    int target = ctx->num_sms * 8;
+    int target = cta_target(ctx);
     int nchunks = target / ngroups;
     if (nchunks < 1) nchunks = 1;
     if (nchunks > a.nwaves) nchunks = a.nwaves;
     a.wpc = (a.nwaves + nchunks - 1) / nchunks;
     nchunks = (a.nwaves + a.wpc - 1) / a.wpc;
-    size_t smem = (size_t)2 * N * C::WC * sizeof(float2) + (C::TWREG ? 0 : (size_t)N * sizeof(float2));
+    size_t smem = (size_t)(2 * exch_elems(N, C::WC) + N * C::WC) * sizeof(float2) + (C::TWREG ? 0 : (size_t)N * sizeof(float2));
     auto kern = k_col<N, MODE>;
     if (smem > 48 * 1024) TACAW_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     kern<<<dim3(ngroups, nchunks), C::THREADS, smem, st>>>(a);

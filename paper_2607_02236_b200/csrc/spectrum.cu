@@ -30,17 +30,18 @@ __global__ void __launch_bounds__(SpecCfg<N>::THREADS) k_spectrum(const float2* 
     constexpr int E = C::E, T = C::T, WQ = C::WQ;
     constexpr bool TWREG = C::TWREG;
     using P = FftPlan<N, E>;
-    extern __shared__ float2 smem[];
+    extern __shared__ __align__(16) float2 smem[];
     const int lt = threadIdx.x;
     const int c = lt % WQ, tid = lt / WQ;
+    constexpr int XE = exch_elems(N, WQ);
     float2* smA = smem;
-    float2* smB = smem + (size_t)N * WQ;
+    float2* smB = smem + XE;
     const float2* roots_s = nullptr;
     float2 tw[P::NTW];
     if constexpr (TWREG) {
         TwInit<N, E, 1, 0>::run(tw, roots, tid);
     } else {
-        float2* rs = smem + (size_t)2 * N * WQ;
+        float2* rs = smem + 2 * XE;
         for (int i = lt; i < N; i += blockDim.x) rs[i] = roots[i];
         roots_s = rs;
         __syncthreads();
@@ -57,8 +58,13 @@ __global__ void __launch_bounds__(SpecCfg<N>::THREADS) k_spectrum(const float2* 
         float w = window[f];
         x[m] = make_float2(v.x * w, v.y * w);
     }
-    if constexpr (C::THREADS <= 32) fft_regs<N, E, WQ, false, TWREG>(x, tw, roots_s, smA, smB, tid, c, SyncWarp{});
-    else fft_regs<N, E, WQ, false, TWREG>(x, tw, roots_s, smA, smB, tid, c, SyncBlock{});
+    if constexpr (C::THREADS <= 32) {
+        SyncWarp sync;
+        fft_regs<N, E, WQ, false, TWREG>(x, tw, roots_s, smA, smB, tid, c, sync);
+    } else {
+        SyncBlock sync;
+        fft_regs<N, E, WQ, false, TWREG>(x, tw, roots_s, smA, smB, tid, c, sync);
+    }
     if (!live) return;
     float* dst = I + (size_t)p * nE * (size_t)nroi + r;
 #pragma unroll
@@ -73,7 +79,7 @@ template <int N>
 static int launch_spec_n(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int64_t nroi, const float2* roots,
                          const float* d_window, const float* d_bose, int e_lo, int nE, float* d_I, cudaStream_t st) {
     using C = SpecCfg<N>;
-    size_t smem = (size_t)2 * N * C::WQ * sizeof(float2) + (C::TWREG ? 0 : (size_t)N * sizeof(float2));
+    size_t smem = (size_t)2 * exch_elems(N, C::WQ) * sizeof(float2) + (C::TWREG ? 0 : (size_t)N * sizeof(float2));
     auto kern = k_spectrum<N>;
     if (smem > 48 * 1024) TACAW_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int64_t gx = (nroi + C::WQ - 1) / C::WQ;
