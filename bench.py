@@ -58,6 +58,23 @@ def workload_config(wl, extra=None):
     return c
 
 
+def shard_workload(wl, rank: int):
+    """Rank r works on its own scan batch: the same raster shifted by 0.1 A * r (independent unit)."""
+    if rank > 0:
+        wl.probes_xy = wl.probes_xy + 0.1 * rank
+    return wl
+
+
+def max_over_ranks(value_ms: float, dist, device):
+    """Timing contract: the step time of the job is the slowest rank's."""
+    if dist is None:
+        return value_ms
+    import torch
+    t = torch.tensor([value_ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -170,9 +187,7 @@ def main():
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
-    if rank > 0:
-        # every rank = its own scan batch (other probe positions of the same raster), same size
-        wl.probes_xy = wl.probes_xy + 0.1 * rank
+    shard_workload(wl, rank)          # every rank = its own scan batch of the same size
 
     from paper_2607_02236_b200.pipeline import Runner
     r = Runner(wl, device=local_rank)
@@ -224,10 +239,7 @@ def main():
     elapsed_ms = ev0.elapsed_time(ev1)
     launches = r.tc.launches - l0
     clocks = sampler.stop() if rank == 0 else None
-    if dist is not None:
-        t = torch.tensor([elapsed_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        elapsed_ms = float(t.item())
+    elapsed_ms = max_over_ranks(elapsed_ms, dist, dev)
     total_steps = wl.slice_steps * args.steps * world
     value = total_steps / (elapsed_ms * 1e-3)
 
@@ -272,10 +284,7 @@ def main():
             e2e_step()
         barrier()
         e_ms = (time.perf_counter() - t0) * 1e3
-        if dist is not None:
-            t = torch.tensor([e_ms], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            e_ms = float(t.item())
+        e_ms = max_over_ranks(e_ms, dist, dev)
         e2e = {"value": wl.slice_steps * nrep * world / (e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                "d2h_bytes_per_step": int(d2h), "steps": nrep}
 

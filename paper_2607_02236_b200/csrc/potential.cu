@@ -2,10 +2,10 @@
 //
 // K1 (O2):  V_n[h,k] = sum_s f_s(q^2) sum_{j in (n,s)} exp(-2 pi i (h x_j/lx + k y_j/ly)),
 // f_s(q^2) = sum_{i<4} a_si exp(-b_si q^2), on in-band (h,k) only.  The phase factorises per atom,
-// exp(-2 pi i h u_j) exp(-2 pi i k v_j), so a slice is a rank-K complex outer-product sum; each
-// CTA owns a 64 x 32 (h,k) tile, stages the per-atom phase vectors of a chunk of atoms in shared
-// memory and accumulates 4x2 outputs per thread in registers.  v_n is real, so only k >= 0 is
-// computed and V(-h,-k) = conj V(h,k) is mirrored on store.
+// exp(-2 pi i h u_j) exp(-2 pi i k v_j), so a slice is a rank-K outer-product sum; each CTA owns a
+// 32 x 32 tile of the quadrant h >= 0, k >= 0, stages the per-atom phase vectors of a chunk of atoms
+// in shared memory and accumulates 2x4 points per thread in registers.  v_n is real, so the other
+// three quadrants follow from the same four real sums (see k_potential).
 // Phases use fixed-point fractional coordinates U = round(u 2^32): (h*U mod 2^32) is exact
 // integer arithmetic, then sincospif -- fp32 h*x/L would lose ~4e-4 rad at |h| ~ 1000.
 #include "ctx.h"
@@ -111,9 +111,15 @@ __global__ void k_compact(const int* __restrict__ keys, int natoms, int nkeys_pe
 }
 
 // ---------------------------------------------------------------------------------------- K1
-constexpr int POT_TH = 64;    // h extent of a tile
-constexpr int POT_TK = 32;    // k extent of a tile
-constexpr int POT_CHUNK = 32; // atoms staged per step
+// Quadrant form.  With ex = e^{-2 pi i h u} = a + ib and ey = e^{-2 pi i k v} = c + id,
+//   ex ey       = (ac - bd) + i(ad + bc)   -> V(h, k)
+//   ex conj(ey) = (ac + bd) + i(bc - ad)   -> V(h,-k)
+// and V(-h,-k) = conj V(h,k), V(-h,k) = conj V(h,-k) because v_n is real.  So the four real sums
+// (ac, bd, ad, bc) over the atoms of a slice, for h >= 0 and k >= 0 only, give all four quadrants:
+// 4 FMA per atom per point for 4 points (a direct complex sum is 4 FMA per point).
+constexpr int POT_T = 32;       // tile edge in h and in k
+constexpr int POT_CHUNK = 64;   // atoms staged per step
+constexpr int POT_THREADS = 128;
 
 __device__ __forceinline__ float2 phase_fixed(uint32_t u, int h) {
     // exp(-2 pi i h u/2^32): (h*u mod 2^32) as a signed fraction of a half turn
@@ -123,82 +129,102 @@ __device__ __forceinline__ float2 phase_fixed(uint32_t u, int h) {
     return make_float2(c, -s);
 }
 
-__global__ void __launch_bounds__(256) k_potential(const uint32_t* __restrict__ sx, const uint32_t* __restrict__ sy,
-                                                    const int* __restrict__ offsets, int nspecies,
-                                                    const AbTable ab,
-                                                    const int* __restrict__ kmax_pot, int hmax, int nx, int ny,
-                                                    float inv_lx, float inv_ly, float2* __restrict__ V) {
-    __shared__ float2 ex[POT_CHUNK][POT_TH];
-    __shared__ float2 ey[POT_CHUNK][POT_TK];
+__global__ void __launch_bounds__(POT_THREADS) k_potential(const uint32_t* __restrict__ sx, const uint32_t* __restrict__ sy,
+                                                            const int* __restrict__ offsets, int nspecies, const AbTable ab,
+                                                            const int* __restrict__ kmax_pot, int hmax, int nx, int ny,
+                                                            float inv_lx, float inv_ly, float2* __restrict__ V) {
+    // phases of the staged atoms: ex[r][atom] = e^{-2 pi i (h0+r) u}, built as coarse[r/8] * fine[r%8]
+    __shared__ float2 ex[POT_T][POT_CHUNK + 1];
+    __shared__ float2 ey[POT_T][POT_CHUNK + 1];
+    __shared__ float2 coarse[2][4][POT_CHUNK];
+    __shared__ float2 fine[2][8][POT_CHUNK];
     const int n = blockIdx.z;
-    const int h0 = -hmax + blockIdx.x * POT_TH;
-    const int k0 = blockIdx.y * POT_TK;
-    const int th = threadIdx.x & 15, tk = threadIdx.x >> 4;   // 16 x 16 threads, 4 x 2 outputs each
-    float2 acc[4][2];
-    float2 vsum[4][2];
+    const int h0 = blockIdx.x * POT_T, k0 = blockIdx.y * POT_T;
+    if (h0 > hmax || kmax_pot[h0] < k0) return;        // tile entirely outside the mask
+    const int lt = threadIdx.x;
+    const int th = lt & 15, tk = lt >> 4;             // 16 x 8 threads, 2 (h) x 4 (k) points each
+    float4 acc[2][4], vs[2][4];
 #pragma unroll
-    for (int i = 0; i < 4; ++i)
+    for (int i = 0; i < 2; ++i)
 #pragma unroll
-        for (int j = 0; j < 2; ++j) vsum[i][j] = make_float2(0.f, 0.f);
+        for (int j = 0; j < 4; ++j) vs[i][j] = make_float4(0.f, 0.f, 0.f, 0.f);
     for (int s = 0; s < nspecies; ++s) {
         const int a0 = offsets[n * nspecies + s], a1 = offsets[n * nspecies + s + 1];
         if (a0 == a1) continue;
 #pragma unroll
-        for (int i = 0; i < 4; ++i)
+        for (int i = 0; i < 2; ++i)
 #pragma unroll
-            for (int j = 0; j < 2; ++j) acc[i][j] = make_float2(0.f, 0.f);
+            for (int j = 0; j < 4; ++j) acc[i][j] = make_float4(0.f, 0.f, 0.f, 0.f);
         for (int base = a0; base < a1; base += POT_CHUNK) {
             const int cnt = min(POT_CHUNK, a1 - base);
             __syncthreads();
-            for (int i = threadIdx.x; i < cnt * (POT_TH + POT_TK); i += blockDim.x) {
-                int at = i / (POT_TH + POT_TK), r = i % (POT_TH + POT_TK);
-                if (r < POT_TH) ex[at][r] = phase_fixed(sx[base + at], h0 + r);
-                else ey[at][r - POT_TH] = phase_fixed(sy[base + at], k0 + r - POT_TH);
+            for (int i = lt; i < POT_CHUNK * 24; i += POT_THREADS) {
+                const int at = i % POT_CHUNK, e = i / POT_CHUNK;       // e: axis*12 + table entry
+                if (at < cnt) {
+                    const int axis = e / 12, j = e % 12;
+                    const uint32_t u = axis ? sy[base + at] : sx[base + at];
+                    if (j < 4) coarse[axis][j][at] = phase_fixed(u, (axis ? k0 : h0) + 8 * j);
+                    else fine[axis][j - 4][at] = phase_fixed(u, j - 4);
+                }
             }
             __syncthreads();
+            for (int i = lt; i < POT_CHUNK * 2 * POT_T; i += POT_THREADS) {
+                const int at = i % POT_CHUNK, rr = i / POT_CHUNK;
+                if (at < cnt) {
+                    const int axis = rr / POT_T, r = rr % POT_T;
+                    const float2 cph = coarse[axis][r >> 3][at], fph = fine[axis][r & 7][at];
+                    const float2 ph = make_float2(cph.x * fph.x - cph.y * fph.y, cph.x * fph.y + cph.y * fph.x);
+                    if (axis) ey[r][at] = ph; else ex[r][at] = ph;
+                }
+            }
+            __syncthreads();
+#pragma unroll 4
             for (int at = 0; at < cnt; ++at) {
-                float2 xh[4], yk[2];
+                float2 xh[2], yk[4];
 #pragma unroll
-                for (int i = 0; i < 4; ++i) xh[i] = ex[at][th + 16 * i];
+                for (int i = 0; i < 2; ++i) xh[i] = ex[th + 16 * i][at];
 #pragma unroll
-                for (int j = 0; j < 2; ++j) yk[j] = ey[at][tk + 16 * j];
+                for (int j = 0; j < 4; ++j) yk[j] = ey[tk + 8 * j][at];
 #pragma unroll
-                for (int i = 0; i < 4; ++i)
+                for (int i = 0; i < 2; ++i)
 #pragma unroll
-                    for (int j = 0; j < 2; ++j) {
-                        acc[i][j].x = fmaf(xh[i].x, yk[j].x, fmaf(-xh[i].y, yk[j].y, acc[i][j].x));
-                        acc[i][j].y = fmaf(xh[i].x, yk[j].y, fmaf(xh[i].y, yk[j].x, acc[i][j].y));
+                    for (int j = 0; j < 4; ++j) {
+                        acc[i][j].x = fmaf(xh[i].x, yk[j].x, acc[i][j].x);
+                        acc[i][j].y = fmaf(xh[i].y, yk[j].y, acc[i][j].y);
+                        acc[i][j].z = fmaf(xh[i].x, yk[j].y, acc[i][j].z);
+                        acc[i][j].w = fmaf(xh[i].y, yk[j].x, acc[i][j].w);
                     }
             }
         }
 #pragma unroll
-        for (int i = 0; i < 4; ++i)
+        for (int i = 0; i < 2; ++i)
 #pragma unroll
-            for (int j = 0; j < 2; ++j) {
-                float qx = (float)(h0 + th + 16 * i) * inv_lx, qy = (float)(k0 + tk + 16 * j) * inv_ly;
+            for (int j = 0; j < 4; ++j) {
+                float qx = (float)(h0 + th + 16 * i) * inv_lx, qy = (float)(k0 + tk + 8 * j) * inv_ly;
                 float q2 = qx * qx + qy * qy;
                 float f = 0.f;
 #pragma unroll
                 for (int g = 0; g < 4; ++g) f += ab.a[s][g] * expf(-ab.b[s][g] * q2);
-                vsum[i][j].x = fmaf(f, acc[i][j].x, vsum[i][j].x);
-                vsum[i][j].y = fmaf(f, acc[i][j].y, vsum[i][j].y);
+                vs[i][j].x = fmaf(f, acc[i][j].x, vs[i][j].x);
+                vs[i][j].y = fmaf(f, acc[i][j].y, vs[i][j].y);
+                vs[i][j].z = fmaf(f, acc[i][j].z, vs[i][j].z);
+                vs[i][j].w = fmaf(f, acc[i][j].w, vs[i][j].w);
             }
     }
     float2* Vn = V + (size_t)n * nx * ny;
 #pragma unroll
-    for (int i = 0; i < 4; ++i)
+    for (int i = 0; i < 2; ++i)
 #pragma unroll
-        for (int j = 0; j < 2; ++j) {
-            int h = h0 + th + 16 * i, k = k0 + tk + 16 * j;
-            if (h > hmax || h < -hmax) continue;
-            int ix = (h + nx) % nx;
-            if (k > kmax_pot[ix]) continue;
-            int iy = k;
-            Vn[(size_t)iy * nx + ix] = vsum[i][j];
-            if (k > 0) {
-                int ixm = (nx - ix) % nx, iym = ny - k;
-                Vn[(size_t)iym * nx + ixm] = make_float2(vsum[i][j].x, -vsum[i][j].y);
-            }
+        for (int j = 0; j < 4; ++j) {
+            const int h = h0 + th + 16 * i, k = k0 + tk + 8 * j;
+            if (h > hmax) continue;
+            if (k > kmax_pot[h]) continue;
+            const float ac = vs[i][j].x, bd = vs[i][j].y, ad = vs[i][j].z, bc = vs[i][j].w;
+            const int ixm = (nx - h) % nx, iym = (ny - k) % ny;
+            Vn[(size_t)k * nx + h] = make_float2(ac - bd, ad + bc);
+            if (k > 0) Vn[(size_t)iym * nx + h] = make_float2(ac + bd, bc - ad);
+            if (h > 0) Vn[(size_t)iym * nx + ixm] = make_float2(ac - bd, -(ad + bc));
+            if (h > 0 && k > 0) Vn[(size_t)k * nx + ixm] = make_float2(ac + bd, ad - bc);
         }
 }
 
@@ -241,8 +267,8 @@ int launch_potential(tacaw_ctx* ctx, const double* d_pos, const int32_t* d_speci
         const int total_slices = nframes * nslices;
         for (int z0i = 0; z0i < total_slices; z0i += 65535) {
             int nz = total_slices - z0i < 65535 ? total_slices - z0i : 65535;
-            dim3 grid((2 * hmax + 1 + POT_TH - 1) / POT_TH, (ctx->kmaxmax_pot + 1 + POT_TK - 1) / POT_TK, nz);
-            k_potential<<<grid, 256, 0, st>>>(sx, sy, offsets + (size_t)z0i * nspecies, nspecies, ab, ctx->d_kmax_pot, hmax, nx,
+            dim3 grid((hmax + 1 + POT_T - 1) / POT_T, (ctx->kmaxmax_pot + 1 + POT_T - 1) / POT_T, nz);
+            k_potential<<<grid, POT_THREADS, 0, st>>>(sx, sy, offsets + (size_t)z0i * nspecies, nspecies, ab, ctx->d_kmax_pot, hmax, nx,
                                               ny, (float)(1.0 / ctx->grid.lx_A), (float)(1.0 / ctx->grid.ly_A),
                                               d_V + (size_t)z0i * nx * ny);
             ctx->launches++;

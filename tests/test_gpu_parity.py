@@ -305,6 +305,37 @@ def test_config2_sampled_exit_waves(torch, B, oracle):
     assert _exit_wave_parity(torch, oracle, wl, [0, 101, 255]) <= TOL_WAVE
 
 
+def test_config2_full_size_bench_launch_configuration(torch, B, oracle):
+    """configs[1] at full size exactly as bench.py runs it (all 256 frames in one block, 1024 waves per
+    tacaw_propagate call, batched build): sampled (probe, frame) rows of the time-ordered buffer against
+    exit waves the oracle computes one by one; plus properties that hold at any size."""
+    from oracle import pipeline as OP
+    from paper_2607_02236_b200.pipeline import Runner
+    wl = W.make_workload(2)
+    r = Runner(wl)
+    assert r.fpb == wl.nframes
+    out = r.run()
+    buf = out["buf"].cpu().numpy()
+    frames = [7, 128, 254]
+    ref = OP.exit_waves(wl, frames, output_space=1)
+    for i, f in enumerate(frames):
+        for p in range(wl.nprobes):
+            want = ref[i, p].ravel()[out["roi"]] / np.sqrt(wl.nx * wl.ny)
+            assert rel_l2(buf[p, f], want) <= TOL_WAVE, (p, f)
+    I = out["I"].cpu().numpy()
+    assert I.shape == (wl.nprobes, wl.nframes, out["roi"].size) and np.all(np.isfinite(I)) and np.all(I >= 0)
+    # Parseval of the spectrum normalisation (oracle pin P10) holds for the GPU result at full size
+    E = out["E"]
+    kbt = W.KB_EV_K * 1e3 * wl.temperature_K
+    bose = np.where(E == 0, 1.0, (E / kbt) / (-np.expm1(-E / kbt + (E == 0))))
+    w = 0.5 - 0.5 * np.cos(2 * np.pi * np.arange(wl.nframes) / wl.nframes)
+    for p in range(wl.nprobes):
+        lhs = (I[p] / bose[:, None]).sum()
+        rhs = ((w ** 2)[:, None] * np.abs(buf[p]) ** 2).sum() / (w ** 2).sum()
+        assert abs(lhs - rhs) <= 2e-4 * rhs
+    r.tc.close()
+
+
 def test_config2_reduced_T_spectrum(torch, B, oracle):
     """configs[1] with T' = 32 frames, all four probes, full ROI: spectra parity."""
     from oracle import pipeline as OP
