@@ -86,7 +86,8 @@ struct RowArgs {
     int nseg, seg, slice;          // which t_n this step uses: trans[f*nseg+seg] + slice*ny*nx
     int nwaves, ny;
     int hmax;                      // in-band columns: ix <= hmax || ix >= nx-hmax
-    int wpc;                       // waves per CTA
+    long long nitems;              // (row block, wave) work items; set by the launcher
+    int ipc;                       // items per CTA; set by the launcher
     const float2* roots;
     float scale;                   // ROW_TRANS: sigma/(lx ly)
 };
@@ -95,13 +96,14 @@ struct ColArgs {
     float2* waves;
     int nwaves, nx;
     int hmax;
-    int wpc;
+    long long nitems;              // (column group, wave) work items; set by the launcher
+    int ipc;                       // items per CTA; set by the launcher
     const float2* roots;           // ny-th roots
     const float2* px;
     const float2* py;
     const int* kmax;
     float pscale;                  // multiplies px*py (1 for COL_MID, nx*ny for COL_LASTQ)
-    int all_groups;                // 1: every column group (mask ignored for group selection)
+    int all_groups;                // unused (COL_LASTQ zero-fills the out-of-band groups itself)
 };
 
 int launch_row(tacaw_ctx* ctx, int mode, const RowArgs& a, cudaStream_t st);

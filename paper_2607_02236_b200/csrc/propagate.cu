@@ -17,17 +17,6 @@
 
 namespace tacaw {
 
-// CTAs per launch aimed for (x SM count): a CTA loops over ceil(nwaves/chunks) waves, prefetching the
-// next one while it transforms the current one.  TACAW_CTAS_PER_SM overrides (tuning only).
-static int cta_target(const tacaw_ctx* ctx) {
-    static int per_sm = [] {
-        const char* e = getenv("TACAW_CTAS_PER_SM");
-        int v = e ? atoi(e) : 0;
-        return v > 0 ? v : 4;
-    }();
-    return ctx->num_sms * per_sm;
-}
-
 // ------------------------------------------------------------------------------------------
 template <int N>
 struct RowCfg {
@@ -35,10 +24,11 @@ struct RowCfg {
     static constexpr int T = N / E;
     static constexpr int THREADS = (T > 256) ? T : 256;   // upper bound on the CTA size
     static constexpr bool TWREG = (E == 8);
+    static constexpr int MINB = (E == 8) ? 3 : 1;          // CTAs per SM the register budget is held to
 };
 
 // Barrier functor that, the first time it fires after being armed, also issues the asynchronous
-// prefetch of the next wave (every thread of the group has read the staging buffers by then).
+// prefetch of the next work item (every thread of the group has read the staging buffers by then).
 template <class Base, class Issue>
 struct SyncPrefetch {
     Base base;
@@ -53,8 +43,12 @@ struct SyncPrefetch {
     }
 };
 
+// Work items of a row launch are (row block, wave) pairs, flattened as rb*nwaves + w and dealt out
+// in equal contiguous ranges to a grid that exactly fills the machine (no partial last wave of
+// CTAs).  Consecutive items of a CTA share the row block, so the t_n row is reloaded only when the
+// frame (or the row block) changes.
 template <int N, int MODE>
-__global__ void __launch_bounds__(RowCfg<N>::THREADS) k_row(RowArgs a) {
+__global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MINB) k_row(RowArgs a) {
     using C = RowCfg<N>;
     constexpr int E = C::E, T = C::T;
     constexpr bool TWREG = C::TWREG;
@@ -66,7 +60,6 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS) k_row(RowArgs a) {
     const int lt = threadIdx.x;
     const int g = lt / T, tid = lt % T;
     const int G = blockDim.x / T;
-    const int row = blockIdx.x * G + g;
     float2* smA = smem + (size_t)g * PER_G;
     float2* smB = smA + XE;
     float2* sW = smA + 2 * XE;
@@ -81,10 +74,9 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS) k_row(RowArgs a) {
         roots_s = rs;
         __syncthreads();
     }
-    const int w0 = blockIdx.y * a.wpc;
-    const int w1 = min(w0 + a.wpc, a.nwaves);
+    const long long i0 = (long long)blockIdx.x * a.ipc;
+    const long long i1 = min(i0 + (long long)a.ipc, a.nitems);
     const size_t npix = (size_t)a.ny * N;
-    const size_t rowoff = (size_t)row * N;
     bool inb[E];
 #pragma unroll
     for (int m = 0; m < E; ++m) {
@@ -92,7 +84,7 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS) k_row(RowArgs a) {
         inb[m] = (MODE == ROW_FIRST) || (ix <= a.hmax) || (ix >= N - a.hmax);
     }
     // asynchronous staging (LDGSTS, 16 B chunks): wave row -> sW (in-band chunks only), t row -> sT
-    auto issue = [&](int w, bool with_t) {
+    auto issue_wave = [&](int w, size_t rowoff) {
         const float2* src;
         if constexpr (MODE == ROW_FIRST) src = a.probes ? a.probes + (size_t)a.wave_probe[w] * npix + rowoff
                                                         : a.waves + (size_t)w * npix + rowoff;
@@ -103,53 +95,71 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS) k_row(RowArgs a) {
             const bool p = (MODE == ROW_FIRST) || (ix0 <= a.hmax) || (ix0 + 1 >= N - a.hmax);
             if (p) cp_async16(sW + ix0, src + ix0);
         }
-        if constexpr (HAS_T) {
-            if (with_t) {
-                const float2* tp = a.trans[(size_t)a.wave_frame[w] * a.nseg + a.seg] + (size_t)a.slice * npix + rowoff;
+    };
+    auto issue_t = [&](int f, size_t rowoff) {
+        const float2* tp = a.trans[(size_t)f * a.nseg + a.seg] + (size_t)a.slice * npix + rowoff;
 #pragma unroll
-                for (int j = 0; j < E / 2; ++j) {
-                    const int ix0 = 2 * (tid + T * j);
-                    cp_async16(sT + ix0, tp + ix0);
-                }
-            }
+        for (int j = 0; j < E / 2; ++j) {
+            const int ix0 = 2 * (tid + T * j);
+            cp_async16(sT + ix0, tp + ix0);
         }
-        cp_async_commit();
     };
     auto body = [&](auto base_sync) {
-        int cur_frame = -1;
-        int next_w = w0;
-        bool next_t = true;
-        auto pf = [&]() { issue(next_w, next_t); };
+        int cur_frame = -1, cur_rb = -1;
+        int next_w = 0, next_f = -1;
+        size_t next_rowoff = 0;
+        int phase = 0;      // which prefetch the next barrier hook issues: 0 wave row, 1 t row
+        auto pf = [&]() {
+            if (phase == 0) issue_wave(next_w, next_rowoff);
+            if constexpr (HAS_T) {
+                if ((phase == 1 || MODE == ROW_FIRST) && next_f >= 0) issue_t(next_f, next_rowoff);
+            }
+            cp_async_commit();
+        };
         SyncPrefetch<decltype(base_sync), decltype(pf)> sync{base_sync, pf, false};
-        if (w0 < w1) issue(w0, true);
-        float2 tr[E];
-        for (int w = w0; w < w1; ++w) {
+        if (i0 < i1) {
+            const int rb = (int)(i0 / a.nwaves), w = (int)(i0 - (long long)rb * a.nwaves);
+            const size_t rowoff = (size_t)(rb * G + g) * N;
+            issue_wave(w, rowoff);
+            if constexpr (HAS_T) {
+                cur_frame = a.wave_frame[w];
+                cur_rb = rb;
+                issue_t(cur_frame, rowoff);
+            }
+            cp_async_commit();
+        }
+        for (long long i = i0; i < i1; ++i) {
+            const int rb = (int)(i / a.nwaves), w = (int)(i - (long long)rb * a.nwaves);
+            const size_t rowoff = (size_t)(rb * G + g) * N;
             cp_async_wait_all();
             base_sync();
             float2 x[E];
 #pragma unroll
             for (int m = 0; m < E; ++m) x[m] = inb[m] ? sW[tid + T * m] : make_float2(0.f, 0.f);
-            if constexpr (HAS_T) {
-                const int f = a.wave_frame[w];
-                if (f != cur_frame) {
-#pragma unroll
-                    for (int m = 0; m < E; ++m) tr[m] = sT[tid + T * m];
-                    cur_frame = f;
+            const bool more = (i + 1 < i1);
+            next_f = -1;
+            if (more) {
+                const int rbn = (int)((i + 1) / a.nwaves);
+                next_w = (int)(i + 1 - (long long)rbn * a.nwaves);
+                next_rowoff = (size_t)(rbn * G + g) * N;
+                if constexpr (HAS_T) {
+                    const int f = a.wave_frame[next_w];
+                    if (f != cur_frame || rbn != cur_rb) { next_f = f; cur_frame = f; cur_rb = rbn; }
                 }
-            }
-            if (w + 1 < w1) {
-                next_w = w + 1;
-                if constexpr (HAS_T) next_t = a.wave_frame[w + 1] != cur_frame;
-                sync.armed = true;
             }
             float2* wrow = a.waves + (size_t)w * npix + rowoff;
             if constexpr (MODE != ROW_FIRST) {
+                phase = 0;
+                sync.armed = more;
                 fft_regs<N, E, 1, true, TWREG, MODE == ROW_LAST>(x, tw, roots_s, smA, smB, tid, 0, sync);
                 if constexpr (fft_nexch<N, E>() & 1) { float2* t_ = smA; smA = smB; smB = t_; }
             }
             if constexpr (HAS_T) {
+                // t_n row from the staging buffer; its successor is prefetched only after this use
 #pragma unroll
-                for (int m = 0; m < E; ++m) x[m] = cmul(x[m], tr[m]);
+                for (int m = 0; m < E; ++m) x[m] = cmul(x[m], sT[tid + T * m]);
+                if constexpr (MODE == ROW_FIRST) { phase = 0; sync.armed = more; }
+                else { phase = 1; sync.armed = (next_f >= 0); }
                 fft_regs<N, E, 1, false, TWREG, true>(x, tw, roots_s, smA, smB, tid, 0, sync);
                 if constexpr (fft_nexch<N, E>() & 1) { float2* t_ = smA; smA = smB; smB = t_; }
 #pragma unroll
@@ -177,6 +187,20 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS) k_row(RowArgs a) {
     }
 }
 
+// grid that fills the machine exactly: occupancy x SM count CTAs (or one CTA per item if fewer)
+template <class K>
+static int machine_ctas(const tacaw_ctx* ctx, K kern, int threads, size_t smem, int* cache) {
+    if (*cache == 0) {
+        int per_sm = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem) != cudaSuccess || per_sm < 1) {
+            (void)cudaGetLastError();
+            per_sm = 1;
+        }
+        *cache = per_sm;
+    }
+    return ctx->num_sms * (*cache);
+}
+
 template <int N, int MODE>
 static int launch_row_n(tacaw_ctx* ctx, const RowArgs& a0, cudaStream_t st) {
     using C = RowCfg<N>;
@@ -184,19 +208,25 @@ static int launch_row_n(tacaw_ctx* ctx, const RowArgs& a0, cudaStream_t st) {
     int G = 256 / C::T;
     if (G < 1) G = 1;
     if (G > a.ny) G = a.ny;
-    int threads = G * C::T;
-    int nrb = a.ny / G;
-    int target = cta_target(ctx);
-    int nchunks = target / nrb;
-    if (nchunks < 1) nchunks = 1;
-    if (nchunks > a.nwaves) nchunks = a.nwaves;
-    a.wpc = (a.nwaves + nchunks - 1) / nchunks;
-    nchunks = (a.nwaves + a.wpc - 1) / a.wpc;
+    const int threads = G * C::T;
+    const int nrb = a.ny / G;
     const int per_g = 2 * exch_elems(N, 1) + ((MODE == ROW_FIRST || MODE == ROW_MID) ? 2 : 1) * N;
-    size_t smem = (size_t)G * per_g * sizeof(float2) + (C::TWREG ? 0 : (size_t)N * sizeof(float2));
+    const size_t smem = (size_t)G * per_g * sizeof(float2) + (C::TWREG ? 0 : (size_t)N * sizeof(float2));
     auto kern = k_row<N, MODE>;
-    if (smem > 48 * 1024) TACAW_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    kern<<<dim3(nrb, nchunks), threads, smem, st>>>(a);
+    static bool attr_set = false;
+    if (!attr_set) {
+        if (smem > 48 * 1024) TACAW_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_set = true;
+    }
+    static int occ_cache[4] = {0, 0, 0, 0};     // per CTA size class (G varies only for tiny ny)
+    int* cache = &occ_cache[threads == 256 ? 0 : (threads == 128 ? 1 : (threads == 64 ? 2 : 3))];
+    if (threads != 256 && threads != 128 && threads != 64) *cache = 0;
+    a.nitems = (long long)nrb * a.nwaves;
+    long long ctas = machine_ctas(ctx, kern, threads, smem, cache);
+    if (ctas > a.nitems) ctas = a.nitems;
+    a.ipc = (int)((a.nitems + ctas - 1) / ctas);
+    ctas = (a.nitems + a.ipc - 1) / a.ipc;
+    kern<<<(unsigned)ctas, threads, smem, st>>>(a);
     ctx->launches++;
     TACAW_CUDA(ctx, cudaGetLastError());
     return TACAW_OK;
@@ -236,13 +266,18 @@ struct ColCfg {
     static constexpr int WC = (N >= 512) ? 4 : 8;
     static constexpr int THREADS = T * WC;
     static constexpr bool TWREG = (E == 8);
+    static constexpr bool USE_SP = (E == 8);     // propagator factors in shared memory instead of registers
+    static constexpr int MINB = (E == 8 && THREADS <= 256) ? 3 : 1;
 };
 
+// Work items of a column launch are (column group, wave) pairs, flattened as gi*nwaves + w over the
+// selected groups (the in-band ones, or all of them when hmax covers the grid) and dealt out in equal
+// contiguous ranges to a machine-filling grid, like the row kernel.
 template <int N, int MODE>
-__global__ void __launch_bounds__(ColCfg<N>::THREADS) k_col(ColArgs a) {
+__global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MINB) k_col(ColArgs a) {
     using C = ColCfg<N>;
     constexpr int E = C::E, T = C::T, WC = C::WC;
-    constexpr bool TWREG = C::TWREG;
+    constexpr bool TWREG = C::TWREG, USE_SP = C::USE_SP && (MODE != COL_INV);
     using P = FftPlan<N, E>;
     extern __shared__ __align__(16) float2 smem[];
     const int lt = threadIdx.x;
@@ -250,62 +285,51 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS) k_col(ColArgs a) {
     constexpr int XE = exch_elems(N, WC);
     float2* smA = smem;
     float2* smB = smem + XE;
-    const float2* roots_s = nullptr;
-    // column group of this CTA
-    const int NG = a.nx / WC;
-    int grp = blockIdx.x;
-    bool inband_group = true;
-    {
-        const int nlo = a.hmax / WC + 1;            // groups covering ix in [0, hmax]
-        const int nhi = (a.hmax + WC - 1) / WC;     // groups covering ix in [nx-hmax, nx)
-        if (a.all_groups) {
-            inband_group = (nlo + nhi >= NG) || (grp < nlo) || (grp >= NG - nhi);
-        } else if (nlo + nhi < NG) {
-            grp = (grp < nlo) ? grp : NG - (nlo + nhi - grp);
-        }
-    }
-    const int ix = grp * WC + c;
-    const int w0 = blockIdx.y * a.wpc;
-    const int w1 = min(w0 + a.wpc, a.nwaves);
-    const size_t npix = (size_t)N * a.nx;
-
-    if (MODE == COL_LASTQ && !inband_group) {       // out-of-band columns of Psi_S are exactly zero
-        for (int w = w0; w < w1; ++w) {
-            float2* wc = a.waves + (size_t)w * npix + ix;
-#pragma unroll
-            for (int m = 0; m < E; ++m) wc[(size_t)(tid + T * m) * a.nx] = make_float2(0.f, 0.f);
-        }
-        return;
-    }
-
     float2* sW = smem + 2 * XE;                  // staging tile [N][WC]
+    float2* sP = sW + N * WC;                    // Px Py M /(nx ny) of this CTA's column group (USE_SP)
+    const float2* roots_s = nullptr;
     float2 tw[P::NTW];
     if constexpr (TWREG) {
         TwInit<N, E, 1, 0>::run(tw, a.roots, tid);
     } else {
-        float2* rs = smem + 2 * XE + N * WC;
+        float2* rs = sW + N * WC + (C::USE_SP ? N * WC : 0);
         for (int i = lt; i < N; i += blockDim.x) rs[i] = a.roots[i];
         roots_s = rs;
         __syncthreads();
     }
-    float2 pxy[E];
-    // a column that is entirely outside the mask is never written by the row kernel: do not use it
-    // (it may hold anything, and NaN * 0 would not be 0)
+    const int NG = a.nx / WC;
+    const int nlo = a.hmax / WC + 1;            // groups covering ix in [0, hmax]
+    const int nhi = (a.hmax + WC - 1) / WC;     // groups covering ix in [nx-hmax, nx)
+    const bool all = (nlo + nhi >= NG);
+    auto group_of = [&](int gi) { return (all || gi < nlo) ? gi : NG - (nlo + nhi - gi); };
+    const long long i0 = (long long)blockIdx.x * a.ipc;
+    const long long i1 = min(i0 + (long long)a.ipc, a.nitems);
+    const size_t npix = (size_t)N * a.nx;
+
+    float2 pxy[C::USE_SP ? 1 : E];
     bool col_live = true;
-    if constexpr (MODE != COL_INV) {
-        const float2 px = a.px[ix];
-        const int km = a.kmax[ix];
-        col_live = km >= 0;
+    int cur_grp = -1;
+    // propagator factors of column ix: Px[h] Py[k] M[h,k] pscale.  A column that is entirely outside
+    // the mask is never written by the row kernel: it is not used (NaN * 0 would not be 0).
+    auto load_factors = [&](int grp) {
+        if constexpr (MODE != COL_INV) {
+            const int ix = grp * WC + c;
+            const float2 px = a.px[ix];
+            const int km = a.kmax[ix];
+            col_live = km >= 0;
 #pragma unroll
-        for (int m = 0; m < E; ++m) {
-            int ky = tid + T * m;
-            int k = ky < N / 2 ? ky : N - ky;       // |k|
-            float2 p = cmul(px, a.py[ky]);
-            pxy[m] = (k <= km) ? make_float2(p.x * a.pscale, p.y * a.pscale) : make_float2(0.f, 0.f);
+            for (int m = 0; m < E; ++m) {
+                int ky = tid + T * m;
+                int k = ky < N / 2 ? ky : N - ky;       // |k|
+                float2 p = cmul(px, a.py[ky]);
+                float2 v = (k <= km) ? make_float2(p.x * a.pscale, p.y * a.pscale) : make_float2(0.f, 0.f);
+                if constexpr (USE_SP) sP[ky * WC + c] = v;      // thread-private slot
+                else pxy[m] = v;
+            }
         }
-    }
+    };
     // asynchronous staging of the [N][WC] tile of wave w: 16 B chunks, E/2 per thread
-    auto issue = [&](int w) {
+    auto issue = [&](int w, int grp) {
         const float2* src = a.waves + (size_t)w * npix + (size_t)grp * WC;
 #pragma unroll
         for (int j = 0; j < E / 2; ++j) {
@@ -316,26 +340,37 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS) k_col(ColArgs a) {
         cp_async_commit();
     };
     auto body = [&](auto base_sync) {
-        int next_w = w0;
-        auto pf = [&]() { issue(next_w); };
+        int next_w = 0, next_grp = 0;
+        auto pf = [&]() { issue(next_w, next_grp); };
         SyncPrefetch<decltype(base_sync), decltype(pf)> sync{base_sync, pf, false};
-        if (w0 < w1) issue(w0);
-        for (int w = w0; w < w1; ++w) {
+        if (i0 < i1) {
+            const int gi = (int)(i0 / a.nwaves);
+            issue((int)(i0 - (long long)gi * a.nwaves), group_of(gi));
+        }
+        for (long long i = i0; i < i1; ++i) {
+            const int gi = (int)(i / a.nwaves), w = (int)(i - (long long)gi * a.nwaves);
+            const int grp = group_of(gi);
+            if (grp != cur_grp) { load_factors(grp); cur_grp = grp; }
             cp_async_wait_all();
             base_sync();
-            float2* wc = a.waves + (size_t)w * npix + ix;
+            float2* wc = a.waves + (size_t)w * npix + (size_t)grp * WC + c;
             float2 x[E];
 #pragma unroll
             for (int m = 0; m < E; ++m) x[m] = col_live ? sW[(tid + T * m) * WC + c] : make_float2(0.f, 0.f);
-            if (w + 1 < w1) {
-                next_w = w + 1;
+            if (i + 1 < i1) {
+                const int gn = (int)((i + 1) / a.nwaves);
+                next_w = (int)(i + 1 - (long long)gn * a.nwaves);
+                next_grp = group_of(gn);
                 sync.armed = true;
             }
             if constexpr (MODE != COL_INV) {
                 fft_regs<N, E, WC, false, TWREG>(x, tw, roots_s, smA, smB, tid, c, sync);
                 if constexpr (fft_nexch<N, E>() & 1) { float2* t_ = smA; smA = smB; smB = t_; }
 #pragma unroll
-                for (int m = 0; m < E; ++m) x[m] = cmul(x[m], pxy[m]);
+                for (int m = 0; m < E; ++m) {
+                    if constexpr (USE_SP) x[m] = cmul(x[m], sP[(tid + T * m) * WC + c]);
+                    else x[m] = cmul(x[m], pxy[m]);
+                }
             }
             if constexpr (MODE != COL_LASTQ) {
                 fft_regs<N, E, WC, true, TWREG, true>(x, tw, roots_s, smA, smB, tid, c, sync);
@@ -349,27 +384,49 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS) k_col(ColArgs a) {
     else body(SyncBlock{});
 }
 
+// zero the out-of-band columns [c0, c1) of every row of every wave (exit wave Psi_S, O7)
+__global__ void k_zero_cols(float2* __restrict__ waves, long long nrows, int nx, int c0, int c1) {
+    const int width = (c1 - c0) / 2;      // float4 = two complex values; c0, c1 are even
+    const long long total = nrows * width;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
+        const long long r = i / width;
+        const int j = (int)(i - r * width);
+        reinterpret_cast<float4*>(waves + r * nx + c0)[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+}
+
 template <int N, int MODE>
 static int launch_col_n(tacaw_ctx* ctx, const ColArgs& a0, cudaStream_t st) {
     using C = ColCfg<N>;
     ColArgs a = a0;
     const int NG = a.nx / C::WC;
-    int ngroups = NG;
-    if (!a.all_groups) {
-        int nlo = a.hmax / C::WC + 1, nhi = (a.hmax + C::WC - 1) / C::WC;
-        if (nlo + nhi < NG) ngroups = nlo + nhi;
-    }
-    int target = cta_target(ctx);
-    int nchunks = target / ngroups;
-    if (nchunks < 1) nchunks = 1;
-    if (nchunks > a.nwaves) nchunks = a.nwaves;
-    a.wpc = (a.nwaves + nchunks - 1) / nchunks;
-    nchunks = (a.nwaves + a.wpc - 1) / a.wpc;
-    size_t smem = (size_t)(2 * exch_elems(N, C::WC) + N * C::WC) * sizeof(float2) + (C::TWREG ? 0 : (size_t)N * sizeof(float2));
+    const int nlo = a.hmax / C::WC + 1, nhi = (a.hmax + C::WC - 1) / C::WC;
+    const bool all = nlo + nhi >= NG;
+    const int ngroups = all ? NG : nlo + nhi;
+    const size_t smem = (size_t)(2 * exch_elems(N, C::WC) + (C::USE_SP ? 2 : 1) * N * C::WC) * sizeof(float2) +
+                        (C::TWREG ? 0 : (size_t)N * sizeof(float2));
     auto kern = k_col<N, MODE>;
-    if (smem > 48 * 1024) TACAW_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    kern<<<dim3(ngroups, nchunks), C::THREADS, smem, st>>>(a);
+    static bool attr_set = false;
+    if (!attr_set) {
+        if (smem > 48 * 1024) TACAW_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_set = true;
+    }
+    static int occ_cache = 0;
+    a.nitems = (long long)ngroups * a.nwaves;
+    long long ctas = machine_ctas(ctx, kern, C::THREADS, smem, &occ_cache);
+    if (ctas > a.nitems) ctas = a.nitems;
+    a.ipc = (int)((a.nitems + ctas - 1) / ctas);
+    ctas = (a.nitems + a.ipc - 1) / a.ipc;
+    kern<<<(unsigned)ctas, C::THREADS, smem, st>>>(a);
     ctx->launches++;
+    if (MODE == COL_LASTQ && !all) {
+        const int c0 = nlo * C::WC, c1 = (NG - nhi) * C::WC;
+        const long long nrows = (long long)a.nwaves * N;
+        long long blocks = (nrows * ((c1 - c0) / 2) + 255) / 256;
+        if (blocks > ctx->num_sms * 16) blocks = ctx->num_sms * 16;
+        k_zero_cols<<<(unsigned)blocks, 256, 0, st>>>(a.waves, nrows, a.nx, c0, c1);
+        ctx->launches++;
+    }
     TACAW_CUDA(ctx, cudaGetLastError());
     return TACAW_OK;
 }
