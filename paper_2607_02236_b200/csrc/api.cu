@@ -157,6 +157,7 @@ int tacaw_create(tacaw_ctx** out, const tacaw_grid* grid, const tacaw_beam* beam
         if (km >= 0 && ah > ctx->hmax) ctx->hmax = ah;
         if (kp >= 0 && ah > ctx->hmax_pot) ctx->hmax_pot = ah;
         if (kp > ctx->kmaxmax_pot) ctx->kmaxmax_pot = kp;
+        if (km > ctx->kmaxmax) ctx->kmaxmax = km;
     }
     std::vector<float2> rx, ry;
     make_roots(nx, rx);
@@ -227,7 +228,7 @@ int tacaw_build_slices(tacaw_ctx* ctx, const double* d_pos_A, const int32_t* d_s
     // V(q) -> v(r) -> t = exp(i sigma v):  IFFT_y over the in-band columns, then IFFT_x + exp per row
     ColArgs ca{};
     ca.waves = (float2*)d_trans; ca.nwaves = nframes * nslices; ca.nx = nx; ca.hmax = ctx->hmax_pot; ca.roots = ctx->d_roots_y;
-    ca.px = nullptr; ca.py = nullptr; ca.kmax = ctx->d_kmax_pot; ca.pscale = 1.f; ca.all_groups = 0;
+    ca.px = nullptr; ca.py = nullptr; ca.kmax = ctx->d_kmax_pot; ca.pscale = 1.f; ca.kmaxmax = -1;
     rc = launch_col(ctx, COL_INV, ca, ny, st);
     if (rc) return rc;
     RowArgs ra{};
@@ -318,7 +319,7 @@ int tacaw_make_probes(tacaw_ctx* ctx, const double* probe_xy_A, int nprobes, dou
     if (rc) return rc;
     ColArgs ca{};
     ca.waves = (float2*)d_waves; ca.nwaves = nprobes; ca.nx = nx; ca.hmax = hap; ca.roots = ctx->d_roots_y;
-    ca.kmax = d_kap; ca.pscale = 1.f; ca.all_groups = 0;
+    ca.kmax = d_kap; ca.pscale = 1.f; ca.kmaxmax = -1;
     rc = launch_col(ctx, COL_INV, ca, ny, st);
     if (rc) return rc;
     RowArgs ra{};
@@ -423,7 +424,7 @@ int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, const i
                 ca.waves = ra.waves; ca.nwaves = nw; ca.nx = g.nx; ca.hmax = ctx->hmax; ca.roots = ctx->d_roots_y;
                 ca.px = ctx->d_px; ca.py = ctx->d_py; ca.kmax = ctx->d_kmax;
                 ca.pscale = lastq ? (float)((double)g.nx * (double)g.ny) : 1.f;
-                ca.all_groups = lastq ? 1 : 0;
+                ca.kmaxmax = ctx->kmaxmax;
                 rc = launch_col(ctx, lastq ? COL_LASTQ : COL_MID, ca, g.ny, st);
                 if (rc) return rc;
             }

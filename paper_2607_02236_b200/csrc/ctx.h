@@ -23,6 +23,7 @@ struct tacaw_ctx {
     int hmax = 0;                 // largest |h| with any in-band k  (propagator mask)
     int hmax_pot = 0;             // same for the potential
     int kmaxmax_pot = 0;
+    int kmaxmax = 0;              // largest kmax[ix]
 
     double dz_cached = -1.0;
     float2* d_px = nullptr;  // [nx] exp(-i pi lambda dz h^2/lx^2) / nx
@@ -103,7 +104,7 @@ struct ColArgs {
     const float2* py;
     const int* kmax;
     float pscale;                  // multiplies px*py (1 for COL_MID, nx*ny for COL_LASTQ)
-    int all_groups;                // unused (COL_LASTQ zero-fills the out-of-band groups itself)
+    int kmaxmax;                   // largest kmax[ix] of the masked modes (-1: not applicable)
 };
 
 int launch_row(tacaw_ctx* ctx, int mode, const RowArgs& a, cudaStream_t st);

@@ -1,0 +1,162 @@
+// fft2.cuh -- single-exchange register FFTs for the multislice slice step (sm_100a).
+//
+// The slice-step kernels are bound by the L1TEX unit (shared-memory wavefronts + global tag stage, ncu
+// profiles/r1_*), not by HBM or the FMA pipe, so a transform here moves every element through shared
+// memory as few times as possible: thread `tid` of the T = N/E threads that own a transform holds the
+// E = 32 (N >= 512), 16 (N >= 128) or 8 elements x[tid + T*m]; the first pass is one radix-E DFT in
+// registers, ONE padded shared-memory exchange follows, and the second pass does E/R radix-R DFTs
+// (R = N/E) with twiddles read from a per-thread-slot table in shared memory (a warp that holds two
+// rows reads each twiddle as a broadcast).  N = 2048 = 32*32*2 needs a second exchange.  Ownership is
+// x[tid + T*m] before the first pass and after the last one, so global accesses are coalesced.
+// Complex multiplies are two packed fp32x2 instructions (cmul / cmulc in fft_core.cuh).
+#pragma once
+#include "fft_core.cuh"
+
+namespace tacaw {
+
+// ---------------------------------------------------------------------------------------------
+// 32-point DFT in registers: two 16-point DFTs and one combine stage with W32^k.
+template <bool INV, bool SOUT>
+struct Dft<32, INV, SOUT> {
+    static __device__ __forceinline__ void run(float2 (&v)[32]) {
+        float2 e[16], o[16];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) { e[i] = v[2 * i]; o[i] = v[2 * i + 1]; }
+        Dft<16, INV, false>::run(e);
+        Dft<16, INV, false>::run(o);
+        // cos(pi k/16), k = 0..8
+        constexpr float C[9] = {1.0f, 0.98078528040323044913f, 0.92387953251128675613f, 0.83146961230254523708f,
+                                0.70710678118654752440f, 0.55557023301960222474f, 0.38268343236508977173f,
+                                0.19509032201612826785f, 0.0f};
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+            if (k == 0) {
+                v[0] = cadd(e[0], o[0]);  v[16] = csub(e[0], o[0]);
+            } else if (k == 8) {
+                v[8] = add_mi<INV>(e[8], o[8]);  v[24] = sub_mi<INV>(e[8], o[8]);
+            } else if (k == 4) {      // W = c(1 -+ i)
+                float2 t = add_mi<INV>(o[4], o[4]);
+                v[4] = axpy(C[4], t, e[4]);  v[20] = axpy(-C[4], t, e[4]);
+            } else if (k == 12) {     // W = -c(1 +- i)
+                float2 t = sub_mi<INV>(o[12], o[12]);
+                v[12] = axpy(-C[4], t, e[12]);  v[28] = axpy(C[4], t, e[12]);
+            } else {
+                // forward W32^k = (cos(pi k/16), -sin(pi k/16))
+                const float wr = (k < 8) ? C[k] : -C[16 - k];
+                const float wi = (k < 8) ? C[8 - k] : C[k - 8];
+                float2 t = cmul_dir<INV>(o[k], make_float2(wr, -wi));
+                v[k] = cadd(e[k], t);  v[k + 16] = csub(e[k], t);
+            }
+        }
+    }
+};
+
+// ---------------------------------------------------------------------------------------------
+// Plan: elements per thread and pass structure.
+constexpr __host__ __device__ int fft2_elems(int n) { return n >= 512 ? 32 : (n >= 128 ? 16 : 8); }
+
+template <int N>
+struct Plan2 {
+    static constexpr int E = fft2_elems(N);
+    static constexpr int T = N / E;
+    static_assert(N >= 16 && (N & (N - 1)) == 0 && T >= 1, "unsupported size");
+    static constexpr __host__ __device__ int radix(int ns) { return (N / ns >= E) ? E : (N / ns); }
+    // twiddle slots of the passes from `ns` on: (R-1) per butterfly, E/R butterflies per thread
+    static constexpr __host__ __device__ int slots_from(int ns) {
+        return ns >= N ? 0 : ((ns > 1 ? (radix(ns) - 1) * (E / radix(ns)) : 0) + slots_from(ns * radix(ns)));
+    }
+    static constexpr int NSLOT = slots_from(1);
+    static constexpr int TW_ELEMS = NSLOT * T;     // float2 entries of the shared twiddle table
+};
+
+// Exchange buffer: the pass with Ns = 1 writes E consecutive vector elements per thread; one pad of WC
+// elements per thread makes the half-warp wavefronts of those writes and of the (contiguous) reads
+// bank-conflict free.  Later exchanges (N = 2048 only) are conflict free unpadded.
+constexpr __host__ __device__ int exch2_elems(int n, int wc) { return n * wc + (n / fft2_elems(n)) * wc; }
+
+// Fill the shared twiddle table: entry (slot, tid) = root^(t k N/(Ns R)), k = (tid + b T) mod Ns, for the
+// passes with Ns > 1 in order, butterflies b, inputs t = 1..R-1.  roots[j] = exp(-2 pi i j/N).
+template <int N>
+__device__ __forceinline__ void fft2_fill_twiddles(float2* __restrict__ tab, const float2* __restrict__ roots, int lt,
+                                                   int nthreads) {
+    using P = Plan2<N>;
+    constexpr int T = P::T, E = P::E;
+    for (int i = lt; i < P::TW_ELEMS; i += nthreads) {
+        int slot = i / T;
+        const int tid = i - slot * T;
+        int ns = P::radix(1);     // first pass has no twiddles
+        for (;;) {
+            const int r = P::radix(ns), per = (r - 1) * (E / r);
+            if (slot < per) {
+                const int b = slot / (r - 1), t = slot - b * (r - 1) + 1;
+                const int k = (tid + b * T) & (ns - 1);
+                tab[i] = roots[(t * k * (N / (ns * r))) & (N - 1)];
+                break;
+            }
+            slot -= per;
+            ns *= r;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// The passes.  x: registers.  twp = table + tid.  ex: exchange buffer of exch2_elems(N, WC) float2.
+// (tid, c): transform thread and interleaved-column index.  Sync synchronises the threads that share the
+// buffer.  PRESYNC: also synchronise before writing (the buffer may still be read by a previous exchange).
+template <int N, int WC, bool INV, bool PRESYNC, int NS, int SLOT>
+struct Pass2 {
+    using P = Plan2<N>;
+    static constexpr int E = P::E, T = P::T;
+    static constexpr int R = P::radix(NS);
+    static constexpr int NB = E / R;
+    static constexpr bool LAST = (NS * R == N);
+    static constexpr int NSL = (NS > 1) ? (R - 1) * NB : 0;
+    static constexpr bool PAD = (NS == 1);
+    static_assert(LAST || PAD || NS * WC >= 16, "unpadded exchange would conflict");
+    // pad: +WC elements per block of E*WC (the block one thread writes in the first pass)
+    static constexpr __host__ __device__ int rpad(int m) {     // read offset of element m (tid part excluded)
+        return T * m * WC + (PAD ? ((T >= E) ? (T / E) * m : m / (E / T)) * WC : 0);
+    }
+
+    template <class Sync>
+    static __device__ __forceinline__ void run(float2 (&x)[E], const float2* __restrict__ twp, float2* ex, int tid, int c,
+                                               Sync& sync) {
+        if constexpr (!LAST && PRESYNC) sync();
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+            float2 v[R];
+#pragma unroll
+            for (int t = 0; t < R; ++t) v[t] = x[b + t * NB];
+            if constexpr (NS > 1) {
+#pragma unroll
+                for (int t = 1; t < R; ++t) v[t] = cmul_dir<INV>(v[t], twp[(SLOT + b * (R - 1) + (t - 1)) * T]);
+            }
+            Dft<R, INV, false>::run(v);
+            if constexpr (LAST) {
+#pragma unroll
+                for (int t = 0; t < R; ++t) x[b + t * NB] = v[t];
+            } else {
+                const int jb = tid + b * T, k = jb & (NS - 1);
+                float2* wp = ex + ((jb - k) * R + k) * WC + c + (PAD ? jb * WC : 0);
+#pragma unroll
+                for (int t = 0; t < R; ++t) wp[t * NS * WC] = v[t];
+            }
+        }
+        if constexpr (!LAST) {
+            sync();
+            const float2* rp = ex + tid * WC + c + (PAD && T >= E ? (tid / E) * WC : 0);
+#pragma unroll
+            for (int m = 0; m < E; ++m) x[m] = rp[rpad(m)];
+            Pass2<N, WC, INV, true, NS * R, SLOT + NSL>::run(x, twp, ex, tid, c, sync);
+        }
+    }
+};
+
+// One transform of length N over WC interleaved columns; PRESYNC as above for the first exchange.
+template <int N, int WC, bool INV, bool PRESYNC, class Sync>
+__device__ __forceinline__ void fft2(float2 (&x)[Plan2<N>::E], const float2* __restrict__ twp, float2* ex, int tid, int c,
+                                     Sync& sync) {
+    Pass2<N, WC, INV, PRESYNC, 1, 0>::run(x, twp, ex, tid, c, sync);
+}
+
+}  // namespace tacaw

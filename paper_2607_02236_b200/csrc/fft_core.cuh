@@ -22,12 +22,16 @@ namespace tacaw {
 
 __device__ __forceinline__ float2 cadd(float2 a, float2 b) { return __fadd2_rn(a, b); }
 __device__ __forceinline__ float2 csub(float2 a, float2 b) { return __fadd2_rn(a, make_float2(-b.x, -b.y)); }
+// complex multiply as two packed instructions: FMUL2 with a broadcast scalar operand, then FFMA2 whose
+// first operand is the swapped / half-negated register pair (an operand modifier, no extra MOV)
 __device__ __forceinline__ float2 cmul(float2 a, float2 w) {
-    return make_float2(fmaf(a.x, w.x, -a.y * w.y), fmaf(a.x, w.y, a.y * w.x));
+    float2 r = __fmul2_rn(a, make_float2(w.x, w.x));
+    return __ffma2_rn(make_float2(-a.y, a.x), make_float2(w.y, w.y), r);
 }
 // a * conj(w)
 __device__ __forceinline__ float2 cmulc(float2 a, float2 w) {
-    return make_float2(fmaf(a.x, w.x, a.y * w.y), fmaf(a.y, w.x, -a.x * w.y));
+    float2 r = __fmul2_rn(a, make_float2(w.x, w.x));
+    return __ffma2_rn(make_float2(a.y, -a.x), make_float2(w.y, w.y), r);
 }
 template <bool CONJ>
 __device__ __forceinline__ float2 cmul_dir(float2 a, float2 w) {

@@ -10,184 +10,152 @@
 // ROW_FIRST starts from the r-space entrance wave; ROW_LAST returns to r space; COL_LASTQ stops
 // after the propagator multiply and stores the q-space exit wave Psi_S.  ROW_TRANS / COL_INV are
 // the same transforms used by tacaw_build_slices and tacaw_make_probes.
+//
+// Both kernels are built on the single-exchange transforms of fft2.cuh: ncu shows the slice step bound
+// by L1TEX (shared-memory wavefronts), so each 1D transform crosses shared memory once, wave rows and
+// columns go global <-> registers directly, and only what is reused (the t_n rows shared by the probes
+// of a frame, the Py table, the twiddles) is kept in shared memory.
 #include <cstdlib>
 
 #include "ctx.h"
-#include "fft_core.cuh"
+#include "fft2.cuh"
 
 namespace tacaw {
+
+// Which of a thread's elements x[tid + T*m] are inside the band |h| <= H (index <= H or >= N - H).
+// BAND: H = N/3 exactly (square cell with the 2/3 mask) -- the structure is known at compile time:
+// chunks m < M_LO and m > M_HI are inside, chunks between are outside, the two edge chunks depend on
+// tid only.  Otherwise H is a run-time value and every element is tested.
+template <int N, int T, bool BAND>
+struct Band {
+    static constexpr int H = N / 3;
+    static constexpr int M_LO = H / T, M_HI = (N - H) / T;
+    bool lo_ok, hi_ok;
+    int h;
+    __device__ __forceinline__ Band(int tid, int hrun) : lo_ok(tid <= H - T * M_LO), hi_ok(tid >= (N - H) - T * M_HI), h(hrun) {}
+    // compile-time "certainly outside"
+    static constexpr __host__ __device__ bool never(int m) { return BAND && m > M_LO && m < M_HI; }
+    __device__ __forceinline__ bool in(int m, int tid) const {
+        if constexpr (BAND) {
+            return (m < M_LO) || (m > M_HI) || (m == M_LO && lo_ok) || (m == M_HI && hi_ok);
+        } else {
+            const int ix = tid + T * m;
+            return ix <= h || ix >= N - h;
+        }
+    }
+};
 
 // ------------------------------------------------------------------------------------------
 template <int N>
 struct RowCfg {
-    static constexpr int E = (N >= 1024) ? 16 : 8;
-    static constexpr int T = N / E;
-    static constexpr int THREADS = (T > 256) ? T : 256;   // upper bound on the CTA size
-    static constexpr bool TWREG = (E == 8);
-    static constexpr int MINB = (E == 8) ? 3 : 1;          // CTAs per SM the register budget is held to
-};
-
-// Barrier functor that, the first time it fires after being armed, also issues the asynchronous
-// prefetch of the next work item (every thread of the group has read the staging buffers by then).
-template <class Base, class Issue>
-struct SyncPrefetch {
-    Base base;
-    Issue issue;
-    bool armed;
-    __device__ __forceinline__ void operator()() {
-        base();
-        if (armed) {
-            armed = false;
-            issue();
-        }
+    using P = Plan2<N>;
+    static constexpr int E = P::E, T = P::T;
+    static constexpr int TEAM = (T < 32) ? 32 : T;          // threads that share an exchange buffer
+    static constexpr int RPT = TEAM / T;                    // rows a team transforms at once
+    static constexpr int TEAMS = (N >= 2048) ? 2 : 4;       // teams per CTA
+    static constexpr int THREADS = TEAMS * TEAM;
+    static constexpr int XE = exch2_elems(N, 1);            // exchange elements per row
+    static constexpr int MINB = (N >= 2048) ? 1 : 3;
+    static constexpr size_t smem(bool has_t) {
+        return sizeof(float2) * ((size_t)P::TW_ELEMS + (size_t)TEAMS * RPT * (XE + (has_t ? N : 0)));
     }
 };
 
-// Work items of a row launch are (row block, wave) pairs, flattened as rb*nwaves + w and dealt out
-// in equal contiguous ranges to a grid that exactly fills the machine (no partial last wave of
-// CTAs).  Consecutive items of a CTA share the row block, so the t_n row is reloaded only when the
-// frame (or the row block) changes.
-template <int N, int MODE>
+// Work items of a row launch are (row block of RPT rows, wave) pairs, flattened as rb*nwaves + w and
+// dealt out in equal contiguous ranges to the teams of a grid that fills the machine.  Consecutive items
+// of a team share the row block, so its t_n rows are reloaded only when the frame (or block) changes.
+template <int N, int MODE, bool BAND>
 __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MINB) k_row(RowArgs a) {
     using C = RowCfg<N>;
-    constexpr int E = C::E, T = C::T;
-    constexpr bool TWREG = C::TWREG;
+    using P = Plan2<N>;
+    constexpr int E = C::E, T = C::T, TEAM = C::TEAM, RPT = C::RPT;
     constexpr bool HAS_T = (MODE == ROW_FIRST || MODE == ROW_MID);
-    constexpr int XE = exch_elems(N, 1);
-    constexpr int PER_G = 2 * XE + (HAS_T ? 2 : 1) * N;     // exchange A, exchange B, wave stage, t stage
-    using P = FftPlan<N, E>;
     extern __shared__ __align__(16) float2 smem[];
     const int lt = threadIdx.x;
-    const int g = lt / T, tid = lt % T;
-    const int G = blockDim.x / T;
-    float2* smA = smem + (size_t)g * PER_G;
-    float2* smB = smA + XE;
-    float2* sW = smA + 2 * XE;
-    float2* sT = sW + N;
-    const float2* roots_s = nullptr;
-    float2 tw[P::NTW];
-    if constexpr (TWREG) {
-        TwInit<N, E, 1, 0>::run(tw, a.roots, tid);
-    } else {
-        float2* rs = smem + (size_t)G * PER_G;
-        for (int i = lt; i < N; i += blockDim.x) rs[i] = a.roots[i];
-        roots_s = rs;
-        __syncthreads();
-    }
-    const long long i0 = (long long)blockIdx.x * a.ipc;
+    const int team = lt / TEAM, l = lt % TEAM;
+    const int g = l / T, tid = l % T;
+    float2* tw = smem;
+    float2* ex = smem + P::TW_ELEMS + (size_t)team * RPT * (C::XE + (HAS_T ? N : 0)) + (size_t)g * C::XE;
+    float2* sT = smem + P::TW_ELEMS + (size_t)team * RPT * (C::XE + (HAS_T ? N : 0)) + (size_t)RPT * C::XE;   // [RPT][N]
+    fft2_fill_twiddles<N>(tw, a.roots, lt, C::THREADS);
+    __syncthreads();
+    const float2* twp = tw + tid;
+    const Band<N, T, BAND> band(tid, a.hmax);
+
+    const long long gteam = (long long)blockIdx.x * C::TEAMS + team;
+    long long i0 = gteam * a.ipc;
     const long long i1 = min(i0 + (long long)a.ipc, a.nitems);
+    if (i0 >= i1) return;
     const size_t npix = (size_t)a.ny * N;
-    bool inb[E];
-#pragma unroll
-    for (int m = 0; m < E; ++m) {
-        int ix = tid + T * m;
-        inb[m] = (MODE == ROW_FIRST) || (ix <= a.hmax) || (ix >= N - a.hmax);
-    }
-    // asynchronous staging (LDGSTS, 16 B chunks): wave row -> sW (in-band chunks only), t row -> sT
-    auto issue_wave = [&](int w, size_t rowoff) {
-        const float2* src;
-        if constexpr (MODE == ROW_FIRST) src = a.probes ? a.probes + (size_t)a.wave_probe[w] * npix + rowoff
-                                                        : a.waves + (size_t)w * npix + rowoff;
-        else src = a.waves + (size_t)w * npix + rowoff;
-#pragma unroll
-        for (int j = 0; j < E / 2; ++j) {
-            const int ix0 = 2 * (tid + T * j);
-            const bool p = (MODE == ROW_FIRST) || (ix0 <= a.hmax) || (ix0 + 1 >= N - a.hmax);
-            if (p) cp_async16(sW + ix0, src + ix0);
-        }
-    };
-    auto issue_t = [&](int f, size_t rowoff) {
-        const float2* tp = a.trans[(size_t)f * a.nseg + a.seg] + (size_t)a.slice * npix + rowoff;
-#pragma unroll
-        for (int j = 0; j < E / 2; ++j) {
-            const int ix0 = 2 * (tid + T * j);
-            cp_async16(sT + ix0, tp + ix0);
-        }
-    };
-    auto body = [&](auto base_sync) {
-        int cur_frame = -1, cur_rb = -1;
-        int next_w = 0, next_f = -1;
-        size_t next_rowoff = 0;
-        int phase = 0;      // which prefetch the next barrier hook issues: 0 wave row, 1 t row
-        auto pf = [&]() {
-            if (phase == 0) issue_wave(next_w, next_rowoff);
-            if constexpr (HAS_T) {
-                if ((phase == 1 || MODE == ROW_FIRST) && next_f >= 0) issue_t(next_f, next_rowoff);
-            }
-            cp_async_commit();
-        };
-        SyncPrefetch<decltype(base_sync), decltype(pf)> sync{base_sync, pf, false};
-        if (i0 < i1) {
-            const int rb = (int)(i0 / a.nwaves), w = (int)(i0 - (long long)rb * a.nwaves);
-            const size_t rowoff = (size_t)(rb * G + g) * N;
-            issue_wave(w, rowoff);
-            if constexpr (HAS_T) {
-                cur_frame = a.wave_frame[w];
-                cur_rb = rb;
-                issue_t(cur_frame, rowoff);
-            }
-            cp_async_commit();
-        }
+    int rb = (int)(i0 / a.nwaves);
+    int w = (int)(i0 - (long long)rb * a.nwaves);
+
+    auto body = [&](auto sync) {
+        int cur_f = -1, cur_rb = -1;
         for (long long i = i0; i < i1; ++i) {
-            const int rb = (int)(i / a.nwaves), w = (int)(i - (long long)rb * a.nwaves);
-            const size_t rowoff = (size_t)(rb * G + g) * N;
-            cp_async_wait_all();
-            base_sync();
-            float2 x[E];
+            const size_t rowoff = (size_t)(rb * RPT + g) * N + tid;
+            bool t_pending = false;
+            if constexpr (HAS_T) {
+                const int f = a.wave_frame[w];
+                if (f != cur_f || rb != cur_rb) {
+                    cur_f = f;
+                    cur_rb = rb;
+                    sync();        // every thread of the team is done with the previous rows
+                    const float2* tp = a.trans[(size_t)f * a.nseg + a.seg] + (size_t)a.slice * npix + (size_t)rb * RPT * N;
 #pragma unroll
-            for (int m = 0; m < E; ++m) x[m] = inb[m] ? sW[tid + T * m] : make_float2(0.f, 0.f);
-            const bool more = (i + 1 < i1);
-            next_f = -1;
-            if (more) {
-                const int rbn = (int)((i + 1) / a.nwaves);
-                next_w = (int)(i + 1 - (long long)rbn * a.nwaves);
-                next_rowoff = (size_t)(rbn * G + g) * N;
-                if constexpr (HAS_T) {
-                    const int f = a.wave_frame[next_w];
-                    if (f != cur_frame || rbn != cur_rb) { next_f = f; cur_frame = f; cur_rb = rbn; }
+                    for (int j = 0; j < (RPT * N / 2) / TEAM; ++j) cp_async16(sT + 2 * (l + TEAM * j), tp + 2 * (l + TEAM * j));
+                    cp_async_commit();
+                    t_pending = true;
+                }
+            }
+            float2 x[E];
+            {
+                const float2* src;
+                if constexpr (MODE == ROW_FIRST) src = (a.probes ? a.probes + (size_t)a.wave_probe[w] * npix : a.waves + (size_t)w * npix) + rowoff;
+                else src = a.waves + (size_t)w * npix + rowoff;
+#pragma unroll
+                for (int m = 0; m < E; ++m) {
+                    if (MODE == ROW_FIRST) x[m] = src[T * m];
+                    else if (Band<N, T, BAND>::never(m)) x[m] = make_float2(0.f, 0.f);
+                    else x[m] = band.in(m, tid) ? src[T * m] : make_float2(0.f, 0.f);
                 }
             }
             float2* wrow = a.waves + (size_t)w * npix + rowoff;
-            if constexpr (MODE != ROW_FIRST) {
-                phase = 0;
-                sync.armed = more;
-                fft_regs<N, E, 1, true, TWREG, MODE == ROW_LAST>(x, tw, roots_s, smA, smB, tid, 0, sync);
-                if constexpr (fft_nexch<N, E>() & 1) { float2* t_ = smA; smA = smB; smB = t_; }
-            }
+            if constexpr (MODE != ROW_FIRST) fft2<N, 1, true, true>(x, twp, ex, tid, 0, sync);
             if constexpr (HAS_T) {
-                // t_n row from the staging buffer; its successor is prefetched only after this use
+                if (t_pending) {
+                    cp_async_wait_all();
+                    sync();
+                }
+                const float2* st = sT + g * N + tid;
 #pragma unroll
-                for (int m = 0; m < E; ++m) x[m] = cmul(x[m], sT[tid + T * m]);
-                if constexpr (MODE == ROW_FIRST) { phase = 0; sync.armed = more; }
-                else { phase = 1; sync.armed = (next_f >= 0); }
-                fft_regs<N, E, 1, false, TWREG, true>(x, tw, roots_s, smA, smB, tid, 0, sync);
-                if constexpr (fft_nexch<N, E>() & 1) { float2* t_ = smA; smA = smB; smB = t_; }
+                for (int m = 0; m < E; ++m) x[m] = cmul(x[m], st[T * m]);
+                fft2<N, 1, false, true>(x, twp, ex, tid, 0, sync);
 #pragma unroll
-                for (int m = 0; m < E; ++m)
-                    if (MODE == ROW_FIRST ? ((tid + T * m <= a.hmax) || (tid + T * m >= N - a.hmax)) : inb[m])
-                        wrow[tid + T * m] = x[m];
+                for (int m = 0; m < E; ++m) {
+                    if (!Band<N, T, BAND>::never(m)) {
+                        if (band.in(m, tid)) wrow[T * m] = x[m];
+                    }
+                }
             } else if constexpr (MODE == ROW_LAST) {
 #pragma unroll
-                for (int m = 0; m < E; ++m) wrow[tid + T * m] = x[m];
+                for (int m = 0; m < E; ++m) wrow[T * m] = x[m];
             } else {  // ROW_TRANS: t = exp(i sigma v), v = Re(x)/(lx ly)
 #pragma unroll
                 for (int m = 0; m < E; ++m) {
                     float s, c;
                     sincosf(a.scale * x[m].x, &s, &c);
-                    wrow[tid + T * m] = make_float2(c, s);
+                    wrow[T * m] = make_float2(c, s);
                 }
             }
+            if (++w == a.nwaves) { w = 0; ++rb; }
         }
     };
-    if constexpr (T <= 32) {
-        body(SyncWarp{});
-    } else {
-        if (G == 1) body(SyncBlock{});
-        else body(SyncNamed{1 + g, T});
-    }
+    if constexpr (TEAM == 32) body(SyncWarp{});
+    else body(SyncNamed{1 + team, TEAM});
 }
 
-// grid that fills the machine exactly: occupancy x SM count CTAs (or one CTA per item if fewer)
+// grid that fills the machine exactly: occupancy x SM count CTAs
 template <class K>
 static int machine_ctas(const tacaw_ctx* ctx, K kern, int threads, size_t smem, int* cache) {
     if (*cache == 0) {
@@ -201,35 +169,36 @@ static int machine_ctas(const tacaw_ctx* ctx, K kern, int threads, size_t smem, 
     return ctx->num_sms * (*cache);
 }
 
-template <int N, int MODE>
-static int launch_row_n(tacaw_ctx* ctx, const RowArgs& a0, cudaStream_t st) {
+template <int N, int MODE, bool BAND>
+static int launch_row_nb(tacaw_ctx* ctx, const RowArgs& a0, cudaStream_t st) {
     using C = RowCfg<N>;
     RowArgs a = a0;
-    int G = 256 / C::T;
-    if (G < 1) G = 1;
-    if (G > a.ny) G = a.ny;
-    const int threads = G * C::T;
-    const int nrb = a.ny / G;
-    const int per_g = 2 * exch_elems(N, 1) + ((MODE == ROW_FIRST || MODE == ROW_MID) ? 2 : 1) * N;
-    const size_t smem = (size_t)G * per_g * sizeof(float2) + (C::TWREG ? 0 : (size_t)N * sizeof(float2));
-    auto kern = k_row<N, MODE>;
+    if (a.ny % C::RPT) return fail(ctx, TACAW_E_UNSUPPORTED, "ny must be a multiple of the rows per team");
+    const size_t smem = C::smem(MODE == ROW_FIRST || MODE == ROW_MID);
+    auto kern = k_row<N, MODE, BAND>;
     static bool attr_set = false;
     if (!attr_set) {
         if (smem > 48 * 1024) TACAW_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_set = true;
     }
-    static int occ_cache[4] = {0, 0, 0, 0};     // per CTA size class (G varies only for tiny ny)
-    int* cache = &occ_cache[threads == 256 ? 0 : (threads == 128 ? 1 : (threads == 64 ? 2 : 3))];
-    if (threads != 256 && threads != 128 && threads != 64) *cache = 0;
-    a.nitems = (long long)nrb * a.nwaves;
-    long long ctas = machine_ctas(ctx, kern, threads, smem, cache);
-    if (ctas > a.nitems) ctas = a.nitems;
-    a.ipc = (int)((a.nitems + ctas - 1) / ctas);
-    ctas = (a.nitems + a.ipc - 1) / a.ipc;
-    kern<<<(unsigned)ctas, threads, smem, st>>>(a);
+    static int occ_cache = 0;
+    a.nitems = (long long)(a.ny / C::RPT) * a.nwaves;
+    long long teams = (long long)machine_ctas(ctx, kern, C::THREADS, smem, &occ_cache) * C::TEAMS;
+    if (teams > a.nitems) teams = a.nitems;
+    a.ipc = (int)((a.nitems + teams - 1) / teams);
+    teams = (a.nitems + a.ipc - 1) / a.ipc;
+    const long long ctas = (teams + C::TEAMS - 1) / C::TEAMS;
+    kern<<<(unsigned)ctas, C::THREADS, smem, st>>>(a);
     ctx->launches++;
     TACAW_CUDA(ctx, cudaGetLastError());
     return TACAW_OK;
+}
+
+template <int N, int MODE>
+static int launch_row_n(tacaw_ctx* ctx, const RowArgs& a, cudaStream_t st) {
+    // ROW_FIRST reads a full r-space row; its stores use the band like the others
+    if (a.hmax == N / 3) return launch_row_nb<N, MODE, true>(ctx, a, st);
+    return launch_row_nb<N, MODE, false>(ctx, a, st);
 }
 
 template <int N>
@@ -261,42 +230,43 @@ int launch_row(tacaw_ctx* ctx, int mode, const RowArgs& a, cudaStream_t st) {
 // ------------------------------------------------------------------------------------------
 template <int N>
 struct ColCfg {
-    static constexpr int E = (N >= 1024) ? 16 : 8;
-    static constexpr int T = N / E;
-    static constexpr int WC = (N >= 512) ? 4 : 8;
+    using P = Plan2<N>;
+    static constexpr int E = P::E, T = P::T;
+    static constexpr int WC = (N >= 2048) ? 4 : 8;          // adjacent columns transformed together
     static constexpr int THREADS = T * WC;
-    static constexpr bool TWREG = (E == 8);
-    static constexpr bool USE_SP = (E == 8);     // propagator factors in shared memory instead of registers
-    static constexpr int MINB = (E == 8 && THREADS <= 256) ? 3 : 1;
+    static constexpr bool PING = (N <= 512);                 // two exchange buffers: one barrier per exchange
+    static constexpr int XE = exch2_elems(N, WC);
+    static constexpr int MINB = (N <= 512) ? 3 : (N == 1024 ? 2 : 1);
+    static constexpr size_t smem() { return sizeof(float2) * ((size_t)P::TW_ELEMS + N + (size_t)(PING ? 2 : 1) * XE); }
 };
 
 // Work items of a column launch are (column group, wave) pairs, flattened as gi*nwaves + w over the
 // selected groups (the in-band ones, or all of them when hmax covers the grid) and dealt out in equal
 // contiguous ranges to a machine-filling grid, like the row kernel.
-template <int N, int MODE>
+// BAND: every kmax[ix] <= N/3, so the chunks of k strictly between N/3 and N - N/3 are masked for
+// every column and are neither multiplied nor tested.
+template <int N, int MODE, bool BAND>
 __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MINB) k_col(ColArgs a) {
     using C = ColCfg<N>;
+    using P = Plan2<N>;
     constexpr int E = C::E, T = C::T, WC = C::WC;
-    constexpr bool TWREG = C::TWREG, USE_SP = C::USE_SP && (MODE != COL_INV);
-    using P = FftPlan<N, E>;
+    // two buffers make the barrier before an exchange write unnecessary only when a work item alternates them
+    constexpr bool PRESYNC = !(C::PING && MODE == COL_MID);
     extern __shared__ __align__(16) float2 smem[];
     const int lt = threadIdx.x;
     const int c = lt % WC, tid = lt / WC;
-    constexpr int XE = exch_elems(N, WC);
-    float2* smA = smem;
-    float2* smB = smem + XE;
-    float2* sW = smem + 2 * XE;                  // staging tile [N][WC]
-    float2* sP = sW + N * WC;                    // Px Py M /(nx ny) of this CTA's column group (USE_SP)
-    const float2* roots_s = nullptr;
-    float2 tw[P::NTW];
-    if constexpr (TWREG) {
-        TwInit<N, E, 1, 0>::run(tw, a.roots, tid);
-    } else {
-        float2* rs = sW + N * WC + (C::USE_SP ? N * WC : 0);
-        for (int i = lt; i < N; i += blockDim.x) rs[i] = a.roots[i];
-        roots_s = rs;
-        __syncthreads();
+    float2* tw = smem;
+    float2* sPy = smem + P::TW_ELEMS;             // Py[ky] * pscale
+    float2* exA = sPy + N;
+    float2* exB = C::PING ? exA + C::XE : exA;
+    fft2_fill_twiddles<N>(tw, a.roots, lt, C::THREADS);
+    if constexpr (MODE != COL_INV) {
+        for (int i = lt; i < N; i += C::THREADS) {
+            const float2 p = a.py[i];
+            sPy[i] = make_float2(p.x * a.pscale, p.y * a.pscale);
+        }
     }
+    const float2* twp = tw + tid;
     const int NG = a.nx / WC;
     const int nlo = a.hmax / WC + 1;            // groups covering ix in [0, hmax]
     const int nhi = (a.hmax + WC - 1) / WC;     // groups covering ix in [nx-hmax, nx)
@@ -305,79 +275,55 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MINB) k_col(Col
     const long long i0 = (long long)blockIdx.x * a.ipc;
     const long long i1 = min(i0 + (long long)a.ipc, a.nitems);
     const size_t npix = (size_t)N * a.nx;
+    using B = Band<N, T, BAND>;
 
-    float2 pxy[C::USE_SP ? 1 : E];
-    bool col_live = true;
-    int cur_grp = -1;
-    // propagator factors of column ix: Px[h] Py[k] M[h,k] pscale.  A column that is entirely outside
-    // the mask is never written by the row kernel: it is not used (NaN * 0 would not be 0).
-    auto load_factors = [&](int grp) {
-        if constexpr (MODE != COL_INV) {
-            const int ix = grp * WC + c;
-            const float2 px = a.px[ix];
-            const int km = a.kmax[ix];
-            col_live = km >= 0;
-#pragma unroll
-            for (int m = 0; m < E; ++m) {
-                int ky = tid + T * m;
-                int k = ky < N / 2 ? ky : N - ky;       // |k|
-                float2 p = cmul(px, a.py[ky]);
-                float2 v = (k <= km) ? make_float2(p.x * a.pscale, p.y * a.pscale) : make_float2(0.f, 0.f);
-                if constexpr (USE_SP) sP[ky * WC + c] = v;      // thread-private slot
-                else pxy[m] = v;
-            }
-        }
-    };
-    // asynchronous staging of the [N][WC] tile of wave w: 16 B chunks, E/2 per thread
-    auto issue = [&](int w, int grp) {
-        const float2* src = a.waves + (size_t)w * npix + (size_t)grp * WC;
-#pragma unroll
-        for (int j = 0; j < E / 2; ++j) {
-            const int id = lt + C::THREADS * j;
-            const int r = id / (WC / 2), part = id % (WC / 2);
-            cp_async16(sW + r * WC + 2 * part, src + (size_t)r * a.nx + 2 * part);
-        }
-        cp_async_commit();
-    };
-    auto body = [&](auto base_sync) {
-        int next_w = 0, next_grp = 0;
-        auto pf = [&]() { issue(next_w, next_grp); };
-        SyncPrefetch<decltype(base_sync), decltype(pf)> sync{base_sync, pf, false};
-        if (i0 < i1) {
-            const int gi = (int)(i0 / a.nwaves);
-            issue((int)(i0 - (long long)gi * a.nwaves), group_of(gi));
-        }
+    auto body = [&](auto sync) {
+        sync();                                  // tables visible
+        if (i0 >= i1) return;
+        int gi = (int)(i0 / a.nwaves);
+        int w = (int)(i0 - (long long)gi * a.nwaves);
+        int cur_gi = -1;
+        float2 px = make_float2(0.f, 0.f);
+        int dlo = -1, dhi = -1;                  // |k| <= km  <=>  T*m <= dlo (m < E/2)  or  N - T*m <= dhi (m >= E/2)
+        bool live = true;
+        size_t coloff = 0;
         for (long long i = i0; i < i1; ++i) {
-            const int gi = (int)(i / a.nwaves), w = (int)(i - (long long)gi * a.nwaves);
-            const int grp = group_of(gi);
-            if (grp != cur_grp) { load_factors(grp); cur_grp = grp; }
-            cp_async_wait_all();
-            base_sync();
-            float2* wc = a.waves + (size_t)w * npix + (size_t)grp * WC + c;
-            float2 x[E];
-#pragma unroll
-            for (int m = 0; m < E; ++m) x[m] = col_live ? sW[(tid + T * m) * WC + c] : make_float2(0.f, 0.f);
-            if (i + 1 < i1) {
-                const int gn = (int)((i + 1) / a.nwaves);
-                next_w = (int)(i + 1 - (long long)gn * a.nwaves);
-                next_grp = group_of(gn);
-                sync.armed = true;
-            }
-            if constexpr (MODE != COL_INV) {
-                fft_regs<N, E, WC, false, TWREG>(x, tw, roots_s, smA, smB, tid, c, sync);
-                if constexpr (fft_nexch<N, E>() & 1) { float2* t_ = smA; smA = smB; smB = t_; }
-#pragma unroll
-                for (int m = 0; m < E; ++m) {
-                    if constexpr (USE_SP) x[m] = cmul(x[m], sP[(tid + T * m) * WC + c]);
-                    else x[m] = cmul(x[m], pxy[m]);
+            if (gi != cur_gi) {
+                cur_gi = gi;
+                const int ix = group_of(gi) * WC + c;
+                coloff = (size_t)ix + (size_t)tid * a.nx;
+                if constexpr (MODE != COL_INV) {
+                    // a column entirely outside the mask is never written by the row kernel: it is not
+                    // read (NaN * 0 would not be 0) and comes out as zeros
+                    const int km = a.kmax[ix];
+                    live = km >= 0;
+                    px = a.px[ix];
+                    dlo = km - tid;
+                    dhi = km + tid;
                 }
             }
-            if constexpr (MODE != COL_LASTQ) {
-                fft_regs<N, E, WC, true, TWREG, true>(x, tw, roots_s, smA, smB, tid, c, sync);
-                if constexpr (fft_nexch<N, E>() & 1) { float2* t_ = smA; smA = smB; smB = t_; }
-            }
+            float2* wc = a.waves + (size_t)w * npix + coloff;
+            const size_t rs = (size_t)T * a.nx;
+            float2 x[E];
 #pragma unroll
-            for (int m = 0; m < E; ++m) wc[(size_t)(tid + T * m) * a.nx] = x[m];
+            for (int m = 0; m < E; ++m) x[m] = live ? wc[m * rs] : make_float2(0.f, 0.f);
+            if constexpr (MODE != COL_INV) {
+                fft2<N, WC, false, PRESYNC>(x, twp, exA, tid, c, sync);
+#pragma unroll
+                for (int m = 0; m < E; ++m) {
+                    if (B::never(m)) {
+                        x[m] = make_float2(0.f, 0.f);
+                    } else {
+                        const bool keep = (T * m < N / 2) ? (T * m <= dlo) : (N - T * m <= dhi);
+                        const float2 p = cmul(px, sPy[tid + T * m]);
+                        x[m] = keep ? cmul(x[m], p) : make_float2(0.f, 0.f);
+                    }
+                }
+            }
+            if constexpr (MODE != COL_LASTQ) fft2<N, WC, true, PRESYNC>(x, twp, exB, tid, c, sync);
+#pragma unroll
+            for (int m = 0; m < E; ++m) wc[m * rs] = x[m];
+            if (++w == a.nwaves) { w = 0; ++gi; }
         }
     };
     if constexpr (C::THREADS <= 32) body(SyncWarp{});
@@ -395,17 +341,16 @@ __global__ void k_zero_cols(float2* __restrict__ waves, long long nrows, int nx,
     }
 }
 
-template <int N, int MODE>
-static int launch_col_n(tacaw_ctx* ctx, const ColArgs& a0, cudaStream_t st) {
+template <int N, int MODE, bool BAND>
+static int launch_col_nb(tacaw_ctx* ctx, const ColArgs& a0, cudaStream_t st) {
     using C = ColCfg<N>;
     ColArgs a = a0;
     const int NG = a.nx / C::WC;
     const int nlo = a.hmax / C::WC + 1, nhi = (a.hmax + C::WC - 1) / C::WC;
     const bool all = nlo + nhi >= NG;
     const int ngroups = all ? NG : nlo + nhi;
-    const size_t smem = (size_t)(2 * exch_elems(N, C::WC) + (C::USE_SP ? 2 : 1) * N * C::WC) * sizeof(float2) +
-                        (C::TWREG ? 0 : (size_t)N * sizeof(float2));
-    auto kern = k_col<N, MODE>;
+    const size_t smem = C::smem();
+    auto kern = k_col<N, MODE, BAND>;
     static bool attr_set = false;
     if (!attr_set) {
         if (smem > 48 * 1024) TACAW_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -433,10 +378,12 @@ static int launch_col_n(tacaw_ctx* ctx, const ColArgs& a0, cudaStream_t st) {
 
 template <int N>
 static int launch_col_mode(tacaw_ctx* ctx, int mode, const ColArgs& a, cudaStream_t st) {
+    // COL_INV applies no mask; the masked modes may skip the k chunks no column keeps
+    const bool band = a.kmaxmax >= 0 && a.kmaxmax <= N / 3;
     switch (mode) {
-        case COL_MID: return launch_col_n<N, COL_MID>(ctx, a, st);
-        case COL_LASTQ: return launch_col_n<N, COL_LASTQ>(ctx, a, st);
-        case COL_INV: return launch_col_n<N, COL_INV>(ctx, a, st);
+        case COL_MID: return band ? launch_col_nb<N, COL_MID, true>(ctx, a, st) : launch_col_nb<N, COL_MID, false>(ctx, a, st);
+        case COL_LASTQ: return band ? launch_col_nb<N, COL_LASTQ, true>(ctx, a, st) : launch_col_nb<N, COL_LASTQ, false>(ctx, a, st);
+        case COL_INV: return launch_col_nb<N, COL_INV, false>(ctx, a, st);
     }
     return fail(ctx, TACAW_E_ARG, "bad column mode");
 }
