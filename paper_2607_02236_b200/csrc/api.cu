@@ -6,6 +6,7 @@
 #include <cstring>
 
 #include "ctx.h"
+#include "fft2.cuh"
 
 namespace tacaw {
 
@@ -73,13 +74,10 @@ static bool mask_in_band(int h, int k, const tacaw_grid& g) {
 
 static bool supported_n(int n) { return n >= 16 && n <= 2048 && (n & (n - 1)) == 0; }
 
+// twiddle table of the slice-step transforms of length n (layout: fft2.cuh)
 static void make_roots(int n, std::vector<float2>& out) {
-    out.resize(n);
-    for (int j = 0; j < n; ++j) {
-        // exact octant symmetries are not needed at fp32: fp64 evaluation rounds correctly
-        double ang = -2.0 * M_PI * (double)j / (double)n;
-        out[j] = make_float2((float)std::cos(ang), (float)std::sin(ang));
-    }
+    out.resize(fft2_table_elems(n));
+    fft2_host_table(n, out.data());
 }
 
 static int ensure_propagator(tacaw_ctx* ctx, double dz, cudaStream_t st) {
@@ -162,14 +160,14 @@ int tacaw_create(tacaw_ctx** out, const tacaw_grid* grid, const tacaw_beam* beam
     std::vector<float2> rx, ry;
     make_roots(nx, rx);
     make_roots(ny, ry);
-    bool ok = cudaMalloc(&ctx->d_roots_x, sizeof(float2) * nx) == cudaSuccess &&
-              cudaMalloc(&ctx->d_roots_y, sizeof(float2) * ny) == cudaSuccess &&
+    bool ok = cudaMalloc(&ctx->d_roots_x, sizeof(float2) * rx.size()) == cudaSuccess &&
+              cudaMalloc(&ctx->d_roots_y, sizeof(float2) * ry.size()) == cudaSuccess &&
               cudaMalloc(&ctx->d_kmax, sizeof(int) * nx) == cudaSuccess &&
               cudaMalloc(&ctx->d_kmax_pot, sizeof(int) * nx) == cudaSuccess &&
               cudaMalloc(&ctx->d_px, sizeof(float2) * nx) == cudaSuccess &&
               cudaMalloc(&ctx->d_py, sizeof(float2) * ny) == cudaSuccess;
-    ok = ok && cudaMemcpy(ctx->d_roots_x, rx.data(), sizeof(float2) * nx, cudaMemcpyHostToDevice) == cudaSuccess &&
-         cudaMemcpy(ctx->d_roots_y, ry.data(), sizeof(float2) * ny, cudaMemcpyHostToDevice) == cudaSuccess &&
+    ok = ok && cudaMemcpy(ctx->d_roots_x, rx.data(), sizeof(float2) * rx.size(), cudaMemcpyHostToDevice) == cudaSuccess &&
+         cudaMemcpy(ctx->d_roots_y, ry.data(), sizeof(float2) * ry.size(), cudaMemcpyHostToDevice) == cudaSuccess &&
          cudaMemcpy(ctx->d_kmax, ctx->kmax.data(), sizeof(int) * nx, cudaMemcpyHostToDevice) == cudaSuccess &&
          cudaMemcpy(ctx->d_kmax_pot, ctx->kmax_pot.data(), sizeof(int) * nx, cudaMemcpyHostToDevice) == cudaSuccess;
     ok = ok && cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming) == cudaSuccess;

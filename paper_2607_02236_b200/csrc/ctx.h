@@ -15,8 +15,8 @@ struct tacaw_ctx {
     int num_sms = 148;
     size_t l2_bytes = 0;
 
-    float2* d_roots_x = nullptr;  // exp(-2 pi i j/nx), j < nx
-    float2* d_roots_y = nullptr;  // exp(-2 pi i j/ny)
+    float2* d_roots_x = nullptr;  // twiddle table of the length-nx transforms (fft2.cuh layout)
+    float2* d_roots_y = nullptr;  // same for length ny
     int* d_kmax = nullptr;        // [nx] per column ix: largest |k| inside the band-limit mask, -1 = none
     int* d_kmax_pot = nullptr;    // [nx] same for the potential (Nyquist row/column excluded)
     std::vector<int> kmax, kmax_pot;
@@ -89,7 +89,7 @@ struct RowArgs {
     int hmax;                      // in-band columns: ix <= hmax || ix >= nx-hmax
     long long nitems;              // (row block, wave) work items; set by the launcher
     int ipc;                       // items per CTA; set by the launcher
-    const float2* roots;
+    const float2* roots;           // twiddle table of length-nx transforms
     float scale;                   // ROW_TRANS: sigma/(lx ly)
 };
 
@@ -99,7 +99,7 @@ struct ColArgs {
     int hmax;
     long long nitems;              // (column group, wave) work items; set by the launcher
     int ipc;                       // items per CTA; set by the launcher
-    const float2* roots;           // ny-th roots
+    const float2* roots;           // twiddle table of length-ny transforms
     const float2* px;
     const float2* py;
     const int* kmax;

@@ -10,6 +10,8 @@
 // x[tid + T*m] before the first pass and after the last one, so global accesses are coalesced.
 // Complex multiplies are two packed fp32x2 instructions (cmul / cmulc in fft_core.cuh).
 #pragma once
+#include <cmath>
+
 #include "fft_core.cuh"
 
 namespace tacaw {
@@ -74,29 +76,46 @@ struct Plan2 {
 // bank-conflict free.  Later exchanges (N = 2048 only) are conflict free unpadded.
 constexpr __host__ __device__ int exch2_elems(int n, int wc) { return n * wc + (n / fft2_elems(n)) * wc; }
 
-// Fill the shared twiddle table: entry (slot, tid) = root^(t k N/(Ns R)), k = (tid + b T) mod Ns, for the
-// passes with Ns > 1 in order, butterflies b, inputs t = 1..R-1.  roots[j] = exp(-2 pi i j/N).
-template <int N>
-__device__ __forceinline__ void fft2_fill_twiddles(float2* __restrict__ tab, const float2* __restrict__ roots, int lt,
-                                                   int nthreads) {
-    using P = Plan2<N>;
-    constexpr int T = P::T, E = P::E;
-    for (int i = lt; i < P::TW_ELEMS; i += nthreads) {
-        int slot = i / T;
-        const int tid = i - slot * T;
-        int ns = P::radix(1);     // first pass has no twiddles
-        for (;;) {
-            const int r = P::radix(ns), per = (r - 1) * (E / r);
-            if (slot < per) {
-                const int b = slot / (r - 1), t = slot - b * (r - 1) + 1;
-                const int k = (tid + b * T) & (ns - 1);
-                tab[i] = roots[(t * k * (N / (ns * r))) & (N - 1)];
-                break;
-            }
-            slot -= per;
-            ns *= r;
-        }
+// Twiddle table, entry (slot, tid) = root^(t k N/(Ns R)), k = (tid + b T) mod Ns, for the passes with
+// Ns > 1 in order, butterflies b, inputs t = 1..R-1; root = exp(-2 pi i/N).  Built once per context on the
+// host in fp64 (fft2_host_table), copied to shared memory by every CTA (fft2_load_twiddles).
+inline int fft2_table_elems(int n) {
+    const int e = fft2_elems(n), t = n / e;
+    int slots = 0;
+    for (int ns = e; ns < n;) {
+        const int r = (n / ns >= e) ? e : n / ns;
+        slots += (r - 1) * (e / r);
+        ns *= r;
     }
+    return slots * t;
+}
+template <class F2>
+inline void fft2_host_table(int n, F2* tab) {
+    const int e = fft2_elems(n), T = n / e;
+    int slot0 = 0;
+    for (int ns = e; ns < n;) {
+        const int r = (n / ns >= e) ? e : n / ns;
+        for (int b = 0; b < e / r; ++b)
+            for (int t = 1; t < r; ++t)
+                for (int tid = 0; tid < T; ++tid) {
+                    const int k = (tid + b * T) & (ns - 1);
+                    const long long idx = ((long long)t * k * (n / (ns * r))) % n;
+                    const double ang = -2.0 * 3.14159265358979323846 * (double)idx / (double)n;
+                    F2 v;
+                    v.x = (float)cos(ang);
+                    v.y = (float)sin(ang);
+                    tab[(size_t)(slot0 + b * (r - 1) + (t - 1)) * T + tid] = v;
+                }
+        slot0 += (r - 1) * (e / r);
+        ns *= r;
+    }
+}
+template <int N>
+__device__ __forceinline__ void fft2_load_twiddles(float2* __restrict__ tab, const float2* __restrict__ gtab, int lt,
+                                                   int nthreads) {
+    static_assert(Plan2<N>::TW_ELEMS % 2 == 0, "table is copied in 16-byte chunks");
+    for (int i = lt; i < Plan2<N>::TW_ELEMS / 2; i += nthreads) cp_async16(tab + 2 * i, gtab + 2 * i);
+    cp_async_commit();
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -118,9 +137,11 @@ struct Pass2 {
         return T * m * WC + (PAD ? ((T >= E) ? (T / E) * m : m / (E / T)) * WC : 0);
     }
 
-    template <class Sync>
+    // hook(): called once, right after the registers were refilled from the LAST exchange of the transform
+    // (the buffer is then free as soon as the sharing threads have synchronised)
+    template <class Sync, class Hook>
     static __device__ __forceinline__ void run(float2 (&x)[E], const float2* __restrict__ twp, float2* ex, int tid, int c,
-                                               Sync& sync) {
+                                               Sync& sync, Hook& hook) {
         if constexpr (!LAST && PRESYNC) sync();
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
@@ -143,20 +164,43 @@ struct Pass2 {
             }
         }
         if constexpr (!LAST) {
+            if constexpr (NS == 1) hook.pre();
             sync();
             const float2* rp = ex + tid * WC + c + (PAD && T >= E ? (tid / E) * WC : 0);
 #pragma unroll
             for (int m = 0; m < E; ++m) x[m] = rp[rpad(m)];
-            Pass2<N, WC, INV, true, NS * R, SLOT + NSL>::run(x, twp, ex, tid, c, sync);
+            using Next = Pass2<N, WC, INV, true, NS * R, SLOT + NSL>;
+            if constexpr (Next::LAST) hook();
+            Next::run(x, twp, ex, tid, c, sync, hook);
         }
     }
 };
 
+// Hooks of a transform: pre() runs right before the barrier of the first exchange (after this thread's
+// writes), operator() right after the registers were refilled from the last exchange.
+struct NoHook {
+    __device__ __forceinline__ void pre() const {}
+    __device__ __forceinline__ void operator()() const {}
+};
+template <class Pre, class Post>
+struct Hooks {
+    Pre pre_;
+    Post post_;
+    __device__ __forceinline__ void pre() { pre_(); }
+    __device__ __forceinline__ void operator()() { post_(); }
+};
+
 // One transform of length N over WC interleaved columns; PRESYNC as above for the first exchange.
+template <int N, int WC, bool INV, bool PRESYNC, class Sync, class Hook>
+__device__ __forceinline__ void fft2(float2 (&x)[Plan2<N>::E], const float2* __restrict__ twp, float2* ex, int tid, int c,
+                                     Sync& sync, Hook& hook) {
+    Pass2<N, WC, INV, PRESYNC, 1, 0>::run(x, twp, ex, tid, c, sync, hook);
+}
 template <int N, int WC, bool INV, bool PRESYNC, class Sync>
 __device__ __forceinline__ void fft2(float2 (&x)[Plan2<N>::E], const float2* __restrict__ twp, float2* ex, int tid, int c,
                                      Sync& sync) {
-    Pass2<N, WC, INV, PRESYNC, 1, 0>::run(x, twp, ex, tid, c, sync);
+    NoHook h;
+    Pass2<N, WC, INV, PRESYNC, 1, 0>::run(x, twp, ex, tid, c, sync, h);
 }
 
 }  // namespace tacaw

@@ -64,73 +64,134 @@ struct RowCfg {
 // Work items of a row launch are (row block of RPT rows, wave) pairs, flattened as rb*nwaves + w and
 // dealt out in equal contiguous ranges to the teams of a grid that fills the machine.  Consecutive items
 // of a team share the row block, so its t_n rows are reloaded only when the frame (or block) changes.
+// The rows of the NEXT item are prefetched with cp.async into the team's exchange buffer as soon as the
+// last exchange of the current item has been read back (the buffer is idle during the last pass and
+// the stores), so global latency overlaps arithmetic without a staging buffer of its own.
 template <int N, int MODE, bool BAND>
 __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MINB) k_row(RowArgs a) {
     using C = RowCfg<N>;
     using P = Plan2<N>;
     constexpr int E = C::E, T = C::T, TEAM = C::TEAM, RPT = C::RPT;
     constexpr bool HAS_T = (MODE == ROW_FIRST || MODE == ROW_MID);
+    constexpr bool FULL_IN = (MODE == ROW_FIRST);           // the input row is an r-space row: no band
     extern __shared__ __align__(16) float2 smem[];
     const int lt = threadIdx.x;
     const int team = lt / TEAM, l = lt % TEAM;
     const int g = l / T, tid = l % T;
     float2* tw = smem;
-    float2* ex = smem + P::TW_ELEMS + (size_t)team * RPT * (C::XE + (HAS_T ? N : 0)) + (size_t)g * C::XE;
-    float2* sT = smem + P::TW_ELEMS + (size_t)team * RPT * (C::XE + (HAS_T ? N : 0)) + (size_t)RPT * C::XE;   // [RPT][N]
-    fft2_fill_twiddles<N>(tw, a.roots, lt, C::THREADS);
-    __syncthreads();
+    float2* exw = smem + P::TW_ELEMS + (size_t)team * RPT * (C::XE + (HAS_T ? N : 0));   // team's exchange rows
+    float2* ex = exw + (size_t)g * C::XE;
+    float2* sT = exw + (size_t)RPT * C::XE;                                              // [RPT][N]
+    fft2_load_twiddles<N>(tw, a.roots, lt, C::THREADS);
     const float2* twp = tw + tid;
     const Band<N, T, BAND> band(tid, a.hmax);
 
     const long long gteam = (long long)blockIdx.x * C::TEAMS + team;
-    long long i0 = gteam * a.ipc;
+    const long long i0 = gteam * a.ipc;
     const long long i1 = min(i0 + (long long)a.ipc, a.nitems);
-    if (i0 >= i1) return;
     const size_t npix = (size_t)a.ny * N;
-    int rb = (int)(i0 / a.nwaves);
-    int w = (int)(i0 - (long long)rb * a.nwaves);
+    int rb = 0, w = 0;
+    if (i0 < i1) {
+        rb = (int)(i0 / a.nwaves);
+        w = (int)(i0 - (long long)rb * a.nwaves);
+    }
+    // 16-byte chunks (two elements) of the rows of one item; chunk cch of a row is wanted if it touches the band
+    const int clo = a.hmax / 2, chi = (N - a.hmax) / 2;
+    auto issue_wave = [&](int wv, int rbv) {
+        const float2* src;
+        if constexpr (MODE == ROW_FIRST) src = a.probes ? a.probes + (size_t)a.wave_probe[wv] * npix : a.waves + (size_t)wv * npix;
+        else src = a.waves + (size_t)wv * npix;
+        src += (size_t)rbv * RPT * N;
+        constexpr int NCHR = N / 2, K = RPT * NCHR / TEAM;
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            const int id = l + TEAM * k;
+            const int r = id / NCHR, cch = id % NCHR;
+            bool want = true;
+            if (!FULL_IN) {
+                if (BAND && NCHR % TEAM == 0) {
+                    // cch = l + TEAM*(k % (NCHR/TEAM)): classify the 32-chunk block at compile time
+                    constexpr int CLO = (N / 3) / 2, CHI = (N - N / 3) / 2;
+                    constexpr int BPR = NCHR / TEAM > 0 ? NCHR / TEAM : 1;     // 32-chunk blocks per row
+                    const int lo = TEAM * (k % BPR), hi = lo + TEAM - 1;
+                    if (hi <= CLO || lo >= CHI) want = true;
+                    else if (lo > CLO && hi < CHI) want = false;
+                    else want = (cch <= CLO || cch >= CHI);
+                } else {
+                    want = (cch <= clo || cch >= chi);
+                }
+            }
+            if (want) cp_async16(exw + r * C::XE + 2 * cch, src + (size_t)r * N + 2 * cch);
+        }
+        cp_async_commit();
+    };
 
     auto body = [&](auto sync) {
+        // twiddles (group 0) and the first item's rows (group 1) are in flight together
+        int f_next = 0;
+        if (i0 < i1) {
+            issue_wave(w, rb);
+            if constexpr (HAS_T) f_next = a.wave_frame[w];
+        }
+        cp_async_wait_group<1>();
+        __syncthreads();                          // twiddle table complete (every thread of the CTA gets here)
+        if (i0 >= i1) return;
         int cur_f = -1, cur_rb = -1;
         for (long long i = i0; i < i1; ++i) {
-            const size_t rowoff = (size_t)(rb * RPT + g) * N + tid;
-            bool t_pending = false;
+            bool t_new = false;
             if constexpr (HAS_T) {
-                const int f = a.wave_frame[w];
+                const int f = f_next;
                 if (f != cur_f || rb != cur_rb) {
                     cur_f = f;
                     cur_rb = rb;
-                    sync();        // every thread of the team is done with the previous rows
+                    sync();        // every thread of the team is done with the previous t rows
                     const float2* tp = a.trans[(size_t)f * a.nseg + a.seg] + (size_t)a.slice * npix + (size_t)rb * RPT * N;
 #pragma unroll
                     for (int j = 0; j < (RPT * N / 2) / TEAM; ++j) cp_async16(sT + 2 * (l + TEAM * j), tp + 2 * (l + TEAM * j));
                     cp_async_commit();
-                    t_pending = true;
+                    t_new = true;
                 }
             }
+            // this item's rows: prefetched into the exchange buffer (the t rows, if just issued, may still fly)
+            if (t_new) cp_async_wait_group<1>();
+            else cp_async_wait_all();
+            sync();
             float2 x[E];
-            {
-                const float2* src;
-                if constexpr (MODE == ROW_FIRST) src = (a.probes ? a.probes + (size_t)a.wave_probe[w] * npix : a.waves + (size_t)w * npix) + rowoff;
-                else src = a.waves + (size_t)w * npix + rowoff;
 #pragma unroll
-                for (int m = 0; m < E; ++m) {
-                    if (MODE == ROW_FIRST) x[m] = src[T * m];
-                    else if (Band<N, T, BAND>::never(m)) x[m] = make_float2(0.f, 0.f);
-                    else x[m] = band.in(m, tid) ? src[T * m] : make_float2(0.f, 0.f);
-                }
+            for (int m = 0; m < E; ++m) {
+                if (FULL_IN) x[m] = ex[tid + T * m];
+                else if (Band<N, T, BAND>::never(m)) x[m] = make_float2(0.f, 0.f);
+                else x[m] = band.in(m, tid) ? ex[tid + T * m] : make_float2(0.f, 0.f);
             }
-            float2* wrow = a.waves + (size_t)w * npix + rowoff;
-            if constexpr (MODE != ROW_FIRST) fft2<N, 1, true, true>(x, twp, ex, tid, 0, sync);
+            float2* wrow = a.waves + (size_t)w * npix + (size_t)(rb * RPT + g) * N + tid;
+            // next item
+            int wn = w + 1, rbn = rb;
+            if (wn == a.nwaves) { wn = 0; ++rbn; }
+            const bool more = (i + 1 < i1);
             if constexpr (HAS_T) {
-                if (t_pending) {
+                if (more) f_next = a.wave_frame[wn];
+            }
+            auto post = [&]() {
+                if (more) {
+                    sync();        // every thread of the team has read the exchange back
+                    issue_wave(wn, rbn);
+                }
+            };
+            auto nopre = []() {};
+            Hooks<decltype(nopre), decltype(post)> hook{nopre, post};
+            if constexpr (MODE != ROW_FIRST) {
+                if constexpr (HAS_T) fft2<N, 1, true, true>(x, twp, ex, tid, 0, sync);
+                else fft2<N, 1, true, true>(x, twp, ex, tid, 0, sync, hook);
+            }
+            if constexpr (HAS_T) {
+                if (t_new) {
                     cp_async_wait_all();
                     sync();
                 }
                 const float2* st = sT + g * N + tid;
 #pragma unroll
                 for (int m = 0; m < E; ++m) x[m] = cmul(x[m], st[T * m]);
-                fft2<N, 1, false, true>(x, twp, ex, tid, 0, sync);
+                fft2<N, 1, false, true>(x, twp, ex, tid, 0, sync, hook);
 #pragma unroll
                 for (int m = 0; m < E; ++m) {
                     if (!Band<N, T, BAND>::never(m)) {
@@ -148,7 +209,8 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MINB) k_row(Row
                     wrow[T * m] = make_float2(c, s);
                 }
             }
-            if (++w == a.nwaves) { w = 0; ++rb; }
+            w = wn;
+            rb = rbn;
         }
     };
     if constexpr (TEAM == 32) body(SyncWarp{});
@@ -234,15 +296,16 @@ struct ColCfg {
     static constexpr int E = P::E, T = P::T;
     static constexpr int WC = (N >= 2048) ? 4 : 8;          // adjacent columns transformed together
     static constexpr int THREADS = T * WC;
-    static constexpr bool PING = (N <= 512);                 // two exchange buffers: one barrier per exchange
     static constexpr int XE = exch2_elems(N, WC);
     static constexpr int MINB = (N <= 512) ? 3 : (N == 1024 ? 2 : 1);
-    static constexpr size_t smem() { return sizeof(float2) * ((size_t)P::TW_ELEMS + N + (size_t)(PING ? 2 : 1) * XE); }
+    // twiddles | Py | staging tile [N][WC] | exchange
+    static constexpr size_t smem() { return sizeof(float2) * ((size_t)P::TW_ELEMS + N + (size_t)N * WC + XE); }
 };
 
 // Work items of a column launch are (column group, wave) pairs, flattened as gi*nwaves + w over the
 // selected groups (the in-band ones, or all of them when hmax covers the grid) and dealt out in equal
-// contiguous ranges to a machine-filling grid, like the row kernel.
+// contiguous ranges to a machine-filling grid, like the row kernel.  The [N][WC] tile of the NEXT item is
+// prefetched with cp.async into a staging buffer while the current one is transformed.
 // BAND: every kmax[ix] <= N/3, so the chunks of k strictly between N/3 and N - N/3 are masked for
 // every column and are neither multiplied nor tested.
 template <int N, int MODE, bool BAND>
@@ -250,16 +313,14 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MINB) k_col(Col
     using C = ColCfg<N>;
     using P = Plan2<N>;
     constexpr int E = C::E, T = C::T, WC = C::WC;
-    // two buffers make the barrier before an exchange write unnecessary only when a work item alternates them
-    constexpr bool PRESYNC = !(C::PING && MODE == COL_MID);
     extern __shared__ __align__(16) float2 smem[];
     const int lt = threadIdx.x;
     const int c = lt % WC, tid = lt / WC;
     float2* tw = smem;
     float2* sPy = smem + P::TW_ELEMS;             // Py[ky] * pscale
-    float2* exA = sPy + N;
-    float2* exB = C::PING ? exA + C::XE : exA;
-    fft2_fill_twiddles<N>(tw, a.roots, lt, C::THREADS);
+    float2* sS = sPy + N;                         // staging tile
+    float2* ex = sS + N * WC;
+    fft2_load_twiddles<N>(tw, a.roots, lt, C::THREADS);
     if constexpr (MODE != COL_INV) {
         for (int i = lt; i < N; i += C::THREADS) {
             const float2 p = a.py[i];
@@ -276,12 +337,28 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MINB) k_col(Col
     const long long i1 = min(i0 + (long long)a.ipc, a.nitems);
     const size_t npix = (size_t)N * a.nx;
     using B = Band<N, T, BAND>;
+    // tile of wave wv, column group grp -> staging: 16-byte chunks, E/2 per thread
+    auto issue_tile = [&](int wv, int grp) {
+        const float2* src = a.waves + (size_t)wv * npix + (size_t)grp * WC;
+#pragma unroll
+        for (int j = 0; j < E / 2; ++j) {
+            const int id = lt + C::THREADS * j;
+            const int r = id / (WC / 2), part = id % (WC / 2);
+            cp_async16(sS + r * WC + 2 * part, src + (size_t)r * a.nx + 2 * part);
+        }
+        cp_async_commit();
+    };
 
     auto body = [&](auto sync) {
-        sync();                                  // tables visible
+        int gi = 0, w = 0;
+        if (i0 < i1) {
+            gi = (int)(i0 / a.nwaves);
+            w = (int)(i0 - (long long)gi * a.nwaves);
+            issue_tile(w, group_of(gi));
+        }
+        cp_async_wait_all();
+        sync();                                  // tables and the first tile visible
         if (i0 >= i1) return;
-        int gi = (int)(i0 / a.nwaves);
-        int w = (int)(i0 - (long long)gi * a.nwaves);
         int cur_gi = -1;
         float2 px = make_float2(0.f, 0.f);
         int dlo = -1, dhi = -1;                  // |k| <= km  <=>  T*m <= dlo (m < E/2)  or  N - T*m <= dhi (m >= E/2)
@@ -294,7 +371,7 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MINB) k_col(Col
                 coloff = (size_t)ix + (size_t)tid * a.nx;
                 if constexpr (MODE != COL_INV) {
                     // a column entirely outside the mask is never written by the row kernel: it is not
-                    // read (NaN * 0 would not be 0) and comes out as zeros
+                    // used (NaN * 0 would not be 0) and comes out as zeros
                     const int km = a.kmax[ix];
                     live = km >= 0;
                     px = a.px[ix];
@@ -306,9 +383,14 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MINB) k_col(Col
             const size_t rs = (size_t)T * a.nx;
             float2 x[E];
 #pragma unroll
-            for (int m = 0; m < E; ++m) x[m] = live ? wc[m * rs] : make_float2(0.f, 0.f);
+            for (int m = 0; m < E; ++m) x[m] = live ? sS[(tid + T * m) * WC + c] : make_float2(0.f, 0.f);
+            int wn = w + 1, gn = gi;
+            if (wn == a.nwaves) { wn = 0; ++gn; }
+            const bool more = (i + 1 < i1);
+            sync();                              // staging tile consumed; previous exchange read back
+            if (more) issue_tile(wn, group_of(gn));
             if constexpr (MODE != COL_INV) {
-                fft2<N, WC, false, PRESYNC>(x, twp, exA, tid, c, sync);
+                fft2<N, WC, false, false>(x, twp, ex, tid, c, sync);
 #pragma unroll
                 for (int m = 0; m < E; ++m) {
                     if (B::never(m)) {
@@ -320,10 +402,23 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MINB) k_col(Col
                     }
                 }
             }
-            if constexpr (MODE != COL_LASTQ) fft2<N, WC, true, PRESYNC>(x, twp, exB, tid, c, sync);
+            if constexpr (MODE == COL_MID) {
+                // the barrier inside this exchange also publishes the prefetched tile
+                auto pre = [&]() { cp_async_wait_all(); };
+                NoHook post;
+                Hooks<decltype(pre), NoHook> hooks{pre, post};
+                fft2<N, WC, true, true>(x, twp, ex, tid, c, sync, hooks);
+            } else if constexpr (MODE == COL_INV) {
+                fft2<N, WC, true, false>(x, twp, ex, tid, c, sync);
+            }
 #pragma unroll
             for (int m = 0; m < E; ++m) wc[m * rs] = x[m];
-            if (++w == a.nwaves) { w = 0; ++gi; }
+            if constexpr (MODE != COL_MID) {
+                cp_async_wait_all();
+                sync();                          // prefetched tile visible
+            }
+            w = wn;
+            gi = gn;
         }
     };
     if constexpr (C::THREADS <= 32) body(SyncWarp{});
