@@ -252,10 +252,16 @@ def main():
                 "bytes_per_slice_step": b_step, "peak_source": peak_src,
                 "propagate_share_of_step": prop_ms / elapsed_ms,
                 "propagate_slice_steps_per_s": prop_units / (prop_ms * 1e-3)}
-    tr = os.path.join(ROOT, "profiles", "traffic.json")
+    # dram__bytes_read.sum + dram__bytes_write.sum of the pair from the committed ncu --set full capture, per slice
+    # step like `bytes_per_slice_step`, times the slice steps one tacaw_propagate launch pair covers
+    tr = os.path.join(ROOT, "profiles", "r1_traffic.csv")
     if os.path.exists(tr):
         try:
-            roofline["traffic"] = json.load(open(tr)).get(wl.name)
+            import csv
+            for row in csv.DictReader(open(tr)):
+                if row["workload"] == wl.name:
+                    roofline["traffic"] = float(row["dram_bytes_per_slice_step"])
+                    roofline["traffic_note"] = "bytes per slice step (one wave, row + column kernel), cold-cache ncu capture"
         except Exception:
             pass
 

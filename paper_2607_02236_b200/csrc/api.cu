@@ -354,14 +354,18 @@ int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, const i
     if (rc) return rc;
     const tacaw_grid& g = ctx->grid;
     const size_t npix = (size_t)g.nx * g.ny;
-    // metadata: [wave_frame nwaves][wave_probe nwaves][trans ptrs nframes*nseg]
+    // metadata: [wave_frame nwaves][wave_probe nwaves][tuples <= nwaves*rpt][trans ptrs nframes*nseg]
+    const int rpt = row_tuple_size(g.nx);
     size_t nb_i = sizeof(int) * (size_t)nwaves;
-    size_t off_p = ((2 * nb_i + 15) / 16) * 16;
+    size_t nb_t = sizeof(int) * ((size_t)nwaves + 64) * rpt;
+    size_t off_t = 2 * nb_i;
+    size_t off_p = ((off_t + nb_t + 15) / 16) * 16;
     size_t need = off_p + sizeof(void*) * (size_t)nframes * nsegments + 64;
     rc = ensure(ctx, &ctx->d_meta, &ctx->meta_bytes, need > 4096 ? need : 4096);
     if (rc) return rc;
     int* d_wf = (int*)ctx->d_meta;
     int* d_wp = d_wf + nwaves;
+    int* d_tup = (int*)((char*)ctx->d_meta + off_t);
     const float2** d_tp = (const float2**)((char*)ctx->d_meta + off_p);
     if ((rc = upload(ctx, d_wf, wave_frame, nb_i, st))) return rc;
     if (d_probes && (rc = upload(ctx, d_wp, wave_probe, nb_i, st))) return rc;
@@ -370,7 +374,7 @@ int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, const i
     // depth-first over groups of waves small enough to stay L2-resident between the two kernels of
     // a slice step: all slices for group 0, then group 1, ...
     // a few groups are in flight at once (one per stream)
-    size_t budget = ctx->l2_bytes ? ctx->l2_bytes / 2 : (size_t)64 << 20;
+    size_t budget = ctx->l2_bytes ? ctx->l2_bytes / 4 : (size_t)32 << 20;
     if (const char* e = getenv("TACAW_L2_GROUP_MB")) {
         double mb = atof(e);
         if (mb > 0) budget = (size_t)(mb * 1048576.0);
@@ -380,20 +384,18 @@ int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, const i
     const int ngroups = (nwaves + gmax - 1) / gmax;
     static const int max_streams = [] {
         const char* e = getenv("TACAW_STREAMS");
-        int v = e ? atoi(e) : 2;
+        int v = e ? atoi(e) : 3;
         return v < 1 ? 1 : (v > 1 + tacaw_ctx::MAX_AUX ? 1 + tacaw_ctx::MAX_AUX : v);
     }();
     const int nstreams = ngroups < max_streams ? ngroups : max_streams;
     const bool fork = nstreams >= 2;
     cudaStream_t user_st = st;
-    if (fork) {
-        TACAW_CUDA(ctx, cudaEventRecord(ctx->ev_fork, user_st));
-        for (int i = 0; i + 1 < nstreams; ++i) TACAW_CUDA(ctx, cudaStreamWaitEvent(ctx->aux[i], ctx->ev_fork, 0));
-    }
-    int w0 = 0;
+    // group boundaries (balanced; a boundary moves to the nearest frame change within a quarter group) and the
+    // wave tuples of every group: runs of up to `rpt` consecutive waves of the same frame, indices relative to the
+    // group; a short tuple repeats its last wave
+    std::vector<int> gw(ngroups + 1, 0), tup, tup_off(ngroups + 1, 0);
     for (int gi = 0; gi < ngroups; ++gi) {
-        st = (gi % nstreams) ? ctx->aux[gi % nstreams - 1] : user_st;
-        // balanced groups; a boundary moves to the nearest frame change within a quarter group
+        const int w0 = gw[gi];
         int w1 = (int)(((long long)(gi + 1) * nwaves) / ngroups);
         if (gi + 1 < ngroups) {
             const int slack = (w1 - w0) / 4;
@@ -401,9 +403,27 @@ int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, const i
                 if (w1 + d < nwaves && wave_frame[w1 + d] != wave_frame[w1 + d - 1]) { w1 += d; break; }
                 if (w1 - d > w0 && wave_frame[w1 - d] != wave_frame[w1 - d - 1]) { w1 -= d; break; }
             }
+            if (w1 < w0) w1 = w0;
         } else {
             w1 = nwaves;
         }
+        gw[gi + 1] = w1;
+        for (int w = w0; w < w1;) {
+            int e = w + 1;
+            while (e < w1 && e - w < rpt && wave_frame[e] == wave_frame[w]) ++e;
+            for (int r = 0; r < rpt; ++r) tup.push_back((w + r < e ? w + r : e - 1) - w0);
+            w = e;
+        }
+        tup_off[gi + 1] = (int)(tup.size() / rpt);
+    }
+    if (!tup.empty() && (rc = upload(ctx, d_tup, tup.data(), sizeof(int) * tup.size(), user_st))) return rc;
+    if (fork) {
+        TACAW_CUDA(ctx, cudaEventRecord(ctx->ev_fork, user_st));
+        for (int i = 0; i + 1 < nstreams; ++i) TACAW_CUDA(ctx, cudaStreamWaitEvent(ctx->aux[i], ctx->ev_fork, 0));
+    }
+    for (int gi = 0; gi < ngroups; ++gi) {
+        st = (gi % nstreams) ? ctx->aux[gi % nstreams - 1] : user_st;
+        const int w0 = gw[gi], w1 = gw[gi + 1];
         const int nw = w1 - w0;
         if (nw <= 0) continue;
         int step = 0;
@@ -415,6 +435,8 @@ int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, const i
                 ra.wave_probe = d_wp + w0; ra.wave_frame = d_wf + w0; ra.trans = d_tp;
                 ra.nseg = nsegments; ra.seg = k; ra.slice = n; ra.nwaves = nw; ra.ny = g.ny; ra.hmax = ctx->hmax;
                 ra.roots = ctx->d_roots_x;
+                ra.tuples = d_tup + (size_t)tup_off[gi] * rpt; ra.ntuples = tup_off[gi + 1] - tup_off[gi];
+                ra.pdl = step > 0;      // step 0 may directly follow the kernels that wrote t_n
                 rc = launch_row(ctx, step == 0 ? ROW_FIRST : ROW_MID, ra, st);
                 if (rc) return rc;
                 bool lastq = (step == total - 1) && output_space == 1;
@@ -423,6 +445,7 @@ int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, const i
                 ca.px = ctx->d_px; ca.py = ctx->d_py; ca.kmax = ctx->d_kmax;
                 ca.pscale = lastq ? (float)((double)g.nx * (double)g.ny) : 1.f;
                 ca.kmaxmax = ctx->kmaxmax;
+                ca.pdl = 1;
                 rc = launch_col(ctx, lastq ? COL_LASTQ : COL_MID, ca, g.ny, st);
                 if (rc) return rc;
             }
@@ -431,10 +454,10 @@ int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, const i
             RowArgs ra{};
             ra.waves = (float2*)d_waves + (size_t)w0 * npix; ra.nwaves = nw; ra.ny = g.ny; ra.hmax = ctx->hmax;
             ra.roots = ctx->d_roots_x;
+            ra.pdl = 1;
             rc = launch_row(ctx, ROW_LAST, ra, st);
             if (rc) return rc;
         }
-        w0 = w1;
     }
     if (fork) {
         for (int i = 0; i + 1 < nstreams; ++i) {

@@ -86,8 +86,11 @@ struct RowArgs {
     const float2* const* trans;    // device [nframes*nseg] segment base pointers
     int nseg, seg, slice;          // which t_n this step uses: trans[f*nseg+seg] + slice*ny*nx
     int nwaves, ny;
+    const int* tuples;             // device [ntuples][rows per team] wave indices (same frame within a tuple), or
+    int ntuples;                   //   nullptr: tuple p = waves p*RPT .. (set by the launcher)
+    int pdl;                       // launch as a programmatic dependent of the previous kernel in the stream
     int hmax;                      // in-band columns: ix <= hmax || ix >= nx-hmax
-    long long nitems;              // (row block, wave) work items; set by the launcher
+    long long nitems;              // (row, tuple) work items; set by the launcher
     int ipc;                       // items per CTA; set by the launcher
     const float2* roots;           // twiddle table of length-nx transforms
     float scale;                   // ROW_TRANS: sigma/(lx ly)
@@ -104,10 +107,12 @@ struct ColArgs {
     const float2* py;
     const int* kmax;
     float pscale;                  // multiplies px*py (1 for COL_MID, nx*ny for COL_LASTQ)
+    int pdl;                       // launch as a programmatic dependent of the previous kernel in the stream
     int kmaxmax;                   // largest kmax[ix] of the masked modes (-1: not applicable)
 };
 
 int launch_row(tacaw_ctx* ctx, int mode, const RowArgs& a, cudaStream_t st);
+int row_tuple_size(int nx);        // waves per tuple of the row kernel for this grid width
 int launch_col(tacaw_ctx* ctx, int mode, const ColArgs& a, int ny, cudaStream_t st);
 
 int launch_potential(tacaw_ctx* ctx, const double* d_pos, const int32_t* d_species, int natoms, int nframes, int nspecies,

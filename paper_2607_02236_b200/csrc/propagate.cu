@@ -51,19 +51,21 @@ struct RowCfg {
     using P = Plan2<N>;
     static constexpr int E = P::E, T = P::T;
     static constexpr int TEAM = (T < 32) ? 32 : T;          // threads that share an exchange buffer
-    static constexpr int RPT = TEAM / T;                    // rows a team transforms at once
+    static constexpr int RPT = TEAM / T;                    // rows (one per wave of a tuple) a team transforms at once
     static constexpr int TEAMS = (N >= 2048) ? 2 : 4;       // teams per CTA
     static constexpr int THREADS = TEAMS * TEAM;
     static constexpr int XE = exch2_elems(N, 1);            // exchange elements per row
     static constexpr int MINB = (N >= 2048) ? 1 : 3;
     static constexpr size_t smem(bool has_t) {
-        return sizeof(float2) * ((size_t)P::TW_ELEMS + (size_t)TEAMS * RPT * (XE + (has_t ? N : 0)));
+        return sizeof(float2) * ((size_t)P::TW_ELEMS + (size_t)TEAMS * (RPT * XE + (has_t ? N : 0)));
     }
 };
 
-// Work items of a row launch are (row block of RPT rows, wave) pairs, flattened as rb*nwaves + w and
-// dealt out in equal contiguous ranges to the teams of a grid that fills the machine.  Consecutive items
-// of a team share the row block, so its t_n rows are reloaded only when the frame (or block) changes.
+// A team transforms row y of the RPT waves of a "tuple" at once (RPT = 2 at 256^2 and 512^2: one row per
+// half warp).  The waves of a tuple belong to the same frame, so they share ONE staged t_n row, read
+// back as a broadcast.  Work items are (row, tuple) pairs, flattened as y*ntuples + p and dealt out in
+// equal contiguous ranges to the teams of a grid that fills the machine; consecutive items of a team share
+// the row, so its t_n row is reloaded only when the frame (or the row) changes.
 // The rows of the NEXT item are prefetched with cp.async into the team's exchange buffer as soon as the
 // last exchange of the current item has been read back (the buffer is idle during the last pass and
 // the stores), so global latency overlaps arithmetic without a staging buffer of its own.
@@ -79,9 +81,10 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MINB) k_row(Row
     const int team = lt / TEAM, l = lt % TEAM;
     const int g = l / T, tid = l % T;
     float2* tw = smem;
-    float2* exw = smem + P::TW_ELEMS + (size_t)team * RPT * (C::XE + (HAS_T ? N : 0));   // team's exchange rows
+    float2* exw = smem + P::TW_ELEMS + (size_t)team * (RPT * C::XE + (HAS_T ? N : 0));   // team's exchange rows
     float2* ex = exw + (size_t)g * C::XE;
-    float2* sT = exw + (size_t)RPT * C::XE;                                              // [RPT][N]
+    float2* sT = exw + (size_t)RPT * C::XE;                                              // [N]
+    pdl_launch_dependents();
     fft2_load_twiddles<N>(tw, a.roots, lt, C::THREADS);
     const float2* twp = tw + tid;
     const Band<N, T, BAND> band(tid, a.hmax);
@@ -90,26 +93,56 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MINB) k_row(Row
     const long long i0 = gteam * a.ipc;
     const long long i1 = min(i0 + (long long)a.ipc, a.nitems);
     const size_t npix = (size_t)a.ny * N;
-    int rb = 0, w = 0;
+    int y = 0, p = 0;
     if (i0 < i1) {
-        rb = (int)(i0 / a.nwaves);
-        w = (int)(i0 - (long long)rb * a.nwaves);
+        y = (int)(i0 / a.ntuples);
+        p = (int)(i0 - (long long)y * a.ntuples);
     }
-    // 16-byte chunks (two elements) of the rows of one item; chunk cch of a row is wanted if it touches the band
+    // wave of member r of tuple pv (a short last tuple repeats its last wave: identical work, identical stores)
+    auto member = [&](int pv, int r) {
+        return a.tuples ? __ldg(a.tuples + (size_t)pv * RPT + r) : min(pv * RPT + r, a.nwaves - 1);
+    };
+    // 16-byte chunks (two elements) of the row of every member; chunk cch is wanted if it touches the band
     const int clo = a.hmax / 2, chi = (N - a.hmax) / 2;
-    auto issue_wave = [&](int wv, int rbv) {
-        const float2* src;
-        if constexpr (MODE == ROW_FIRST) src = a.probes ? a.probes + (size_t)a.wave_probe[wv] * npix : a.waves + (size_t)wv * npix;
-        else src = a.waves + (size_t)wv * npix;
-        src += (size_t)rbv * RPT * N;
-        constexpr int NCHR = N / 2, K = RPT * NCHR / TEAM;
+    // RCONST: the member a chunk belongs to is known at compile time (k / (NCHR/TEAM)), so the member waves are
+    // looked up once per item, ahead of time (wm[]); otherwise (tiny grids) each chunk looks its member up
+    constexpr int NCHR = N / 2;
+    constexpr bool RCONST = (NCHR % TEAM == 0);
+    constexpr int NWM = RCONST ? RPT : 1;
+    auto load_members = [&](int pv, int (&wm)[NWM]) {
+        if constexpr (RCONST) {
+#pragma unroll
+            for (int r = 0; r < RPT; ++r) wm[r] = member(pv, r);
+        }
+    };
+    auto own_member = [&](int pv, const int (&wm)[NWM]) {
+        if constexpr (RCONST) {
+            int wv = wm[0];
+#pragma unroll
+            for (int r = 1; r < RPT; ++r) wv = (g == r) ? wm[r] : wv;
+            return wv;
+        } else {
+            return member(pv, g);
+        }
+    };
+    auto issue_wave = [&](int pv, int yv, const int (&wm)[NWM]) {
+        constexpr int K = RPT * NCHR / TEAM;
+        const float2* base[NWM];
+        if constexpr (RCONST) {
+#pragma unroll
+            for (int r = 0; r < RPT; ++r) {
+                if constexpr (MODE == ROW_FIRST) base[r] = a.probes ? a.probes + (size_t)a.wave_probe[wm[r]] * npix : a.waves + (size_t)wm[r] * npix;
+                else base[r] = a.waves + (size_t)wm[r] * npix;
+                base[r] += (size_t)yv * N;
+            }
+        }
 #pragma unroll
         for (int k = 0; k < K; ++k) {
             const int id = l + TEAM * k;
             const int r = id / NCHR, cch = id % NCHR;
             bool want = true;
             if (!FULL_IN) {
-                if (BAND && NCHR % TEAM == 0) {
+                if (BAND && RCONST) {
                     // cch = l + TEAM*(k % (NCHR/TEAM)): classify the 32-chunk block at compile time
                     constexpr int CLO = (N / 3) / 2, CHI = (N - N / 3) / 2;
                     constexpr int BPR = NCHR / TEAM > 0 ? NCHR / TEAM : 1;     // 32-chunk blocks per row
@@ -121,39 +154,71 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MINB) k_row(Row
                     want = (cch <= clo || cch >= chi);
                 }
             }
-            if (want) cp_async16(exw + r * C::XE + 2 * cch, src + (size_t)r * N + 2 * cch);
+            if (want) {
+                const float2* src;
+                if constexpr (RCONST) {
+                    constexpr int BPR = NCHR / TEAM > 0 ? NCHR / TEAM : 1;
+                    src = base[k / BPR];
+                } else {
+                    const int wv = member(pv, r);
+                    if constexpr (MODE == ROW_FIRST) src = a.probes ? a.probes + (size_t)a.wave_probe[wv] * npix : a.waves + (size_t)wv * npix;
+                    else src = a.waves + (size_t)wv * npix;
+                    src += (size_t)yv * N;
+                }
+                cp_async16(exw + r * C::XE + 2 * cch, src + 2 * cch);
+            }
         }
+        cp_async_commit();
+    };
+    auto issue_t = [&](int f, int yv) {
+        const float2* tp = a.trans[(size_t)f * a.nseg + a.seg] + (size_t)a.slice * npix + (size_t)yv * N;
+        constexpr int KT = (N / 2 + TEAM - 1) / TEAM;
+#pragma unroll
+        for (int j = 0; j < KT; ++j)
+            if (N / 2 >= TEAM * KT || l + TEAM * j < N / 2) cp_async16(sT + 2 * (l + TEAM * j), tp + 2 * (l + TEAM * j));
         cp_async_commit();
     };
 
     auto body = [&](auto sync) {
-        // twiddles (group 0) and the first item's rows (group 1) are in flight together
-        int f_next = 0;
+        // nothing before this point reads what the previous kernel of the stream wrote
+        int cur_f = -1, cur_y = -1;
+        int wv = 0, f_next = 0;
+        int wm[NWM] = {0};
+        bool t_new = false;
         if (i0 < i1) {
-            issue_wave(w, rb);
-            if constexpr (HAS_T) f_next = a.wave_frame[w];
+            load_members(p, wm);
+            wv = own_member(p, wm);
+            if constexpr (HAS_T) {
+                // t_n was written long before the previous kernel: stage it while that kernel drains
+                cur_f = a.wave_frame[wv];
+                cur_y = y;
+                issue_t(cur_f, y);
+                t_new = true;
+            }
         }
-        cp_async_wait_group<1>();
+        pdl_wait();
+        if (i0 < i1) issue_wave(p, y, wm);
+        if (i0 >= i1) cp_async_wait_all();                   // twiddles are the oldest group
+        else if (HAS_T) cp_async_wait_group<2>();
+        else cp_async_wait_group<1>();
         __syncthreads();                          // twiddle table complete (every thread of the CTA gets here)
         if (i0 >= i1) return;
-        int cur_f = -1, cur_rb = -1;
         for (long long i = i0; i < i1; ++i) {
-            bool t_new = false;
             if constexpr (HAS_T) {
-                const int f = f_next;
-                if (f != cur_f || rb != cur_rb) {
-                    cur_f = f;
-                    cur_rb = rb;
-                    sync();        // every thread of the team is done with the previous t rows
-                    const float2* tp = a.trans[(size_t)f * a.nseg + a.seg] + (size_t)a.slice * npix + (size_t)rb * RPT * N;
-#pragma unroll
-                    for (int j = 0; j < (RPT * N / 2) / TEAM; ++j) cp_async16(sT + 2 * (l + TEAM * j), tp + 2 * (l + TEAM * j));
-                    cp_async_commit();
-                    t_new = true;
+                if (i > i0) {
+                    const int f = f_next;
+                    t_new = (f != cur_f || y != cur_y);
+                    if (t_new) {
+                        cur_f = f;
+                        cur_y = y;
+                        sync();        // every thread of the team is done with the previous t row
+                        issue_t(f, y);
+                    }
                 }
             }
-            // this item's rows: prefetched into the exchange buffer (the t rows, if just issued, may still fly)
-            if (t_new) cp_async_wait_group<1>();
+            // this item's rows were prefetched into the exchange buffer; a t row issued after them may still fly.
+            // (first item: the t row is older than the rows, both are waited for here)
+            if (t_new && i > i0) cp_async_wait_group<1>();
             else cp_async_wait_all();
             sync();
             float2 x[E];
@@ -163,18 +228,21 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MINB) k_row(Row
                 else if (Band<N, T, BAND>::never(m)) x[m] = make_float2(0.f, 0.f);
                 else x[m] = band.in(m, tid) ? ex[tid + T * m] : make_float2(0.f, 0.f);
             }
-            float2* wrow = a.waves + (size_t)w * npix + (size_t)(rb * RPT + g) * N + tid;
+            float2* wrow = a.waves + (size_t)wv * npix + (size_t)y * N + tid;
             // next item
-            int wn = w + 1, rbn = rb;
-            if (wn == a.nwaves) { wn = 0; ++rbn; }
+            int pn = p + 1, yn = y;
+            if (pn == a.ntuples) { pn = 0; ++yn; }
             const bool more = (i + 1 < i1);
-            if constexpr (HAS_T) {
-                if (more) f_next = a.wave_frame[wn];
+            int wvn = wv;
+            if (more) {
+                load_members(pn, wm);
+                wvn = own_member(pn, wm);
+                if constexpr (HAS_T) f_next = a.wave_frame[wvn];
             }
             auto post = [&]() {
                 if (more) {
                     sync();        // every thread of the team has read the exchange back
-                    issue_wave(wn, rbn);
+                    issue_wave(pn, yn, wm);
                 }
             };
             auto nopre = []() {};
@@ -184,11 +252,11 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MINB) k_row(Row
                 else fft2<N, 1, true, true>(x, twp, ex, tid, 0, sync, hook);
             }
             if constexpr (HAS_T) {
-                if (t_new) {
+                if (t_new && i > i0) {
                     cp_async_wait_all();
                     sync();
                 }
-                const float2* st = sT + g * N + tid;
+                const float2* st = sT + tid;
 #pragma unroll
                 for (int m = 0; m < E; ++m) x[m] = cmul(x[m], st[T * m]);
                 fft2<N, 1, false, true>(x, twp, ex, tid, 0, sync, hook);
@@ -209,12 +277,34 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MINB) k_row(Row
                     wrow[T * m] = make_float2(c, s);
                 }
             }
-            w = wn;
-            rb = rbn;
+            p = pn;
+            y = yn;
+            wv = wvn;
         }
     };
     if constexpr (TEAM == 32) body(SyncWarp{});
     else body(SyncNamed{1 + team, TEAM});
+}
+
+// Launch with programmatic dependent launch when asked: the kernel may start while its predecessor in the
+// stream drains; everything it does before pdl_wait() must not depend on that predecessor.
+template <class K, class A>
+static cudaError_t launch_pdl(K kern, unsigned grid, int threads, size_t smem, cudaStream_t st, bool pdl, const A& a) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(threads);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    static const bool pdl_on = [] {
+        const char* e = getenv("TACAW_PDL");
+        return e ? atoi(e) != 0 : true;
+    }();
+    cfg.numAttrs = (pdl && pdl_on) ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, a);
 }
 
 // grid that fills the machine exactly: occupancy x SM count CTAs
@@ -235,7 +325,7 @@ template <int N, int MODE, bool BAND>
 static int launch_row_nb(tacaw_ctx* ctx, const RowArgs& a0, cudaStream_t st) {
     using C = RowCfg<N>;
     RowArgs a = a0;
-    if (a.ny % C::RPT) return fail(ctx, TACAW_E_UNSUPPORTED, "ny must be a multiple of the rows per team");
+    if (!a.tuples) a.ntuples = (a.nwaves + C::RPT - 1) / C::RPT;
     const size_t smem = C::smem(MODE == ROW_FIRST || MODE == ROW_MID);
     auto kern = k_row<N, MODE, BAND>;
     static bool attr_set = false;
@@ -244,13 +334,13 @@ static int launch_row_nb(tacaw_ctx* ctx, const RowArgs& a0, cudaStream_t st) {
         attr_set = true;
     }
     static int occ_cache = 0;
-    a.nitems = (long long)(a.ny / C::RPT) * a.nwaves;
+    a.nitems = (long long)a.ny * a.ntuples;
     long long teams = (long long)machine_ctas(ctx, kern, C::THREADS, smem, &occ_cache) * C::TEAMS;
     if (teams > a.nitems) teams = a.nitems;
     a.ipc = (int)((a.nitems + teams - 1) / teams);
     teams = (a.nitems + a.ipc - 1) / a.ipc;
     const long long ctas = (teams + C::TEAMS - 1) / C::TEAMS;
-    kern<<<(unsigned)ctas, C::THREADS, smem, st>>>(a);
+    TACAW_CUDA(ctx, launch_pdl(kern, (unsigned)ctas, C::THREADS, smem, st, a.pdl != 0, a));
     ctx->launches++;
     TACAW_CUDA(ctx, cudaGetLastError());
     return TACAW_OK;
@@ -274,6 +364,11 @@ static int launch_row_mode(tacaw_ctx* ctx, int mode, const RowArgs& a, cudaStrea
     return fail(ctx, TACAW_E_ARG, "bad row mode");
 }
 
+int row_tuple_size(int nx) {
+    const int t = nx / fft2_elems(nx);
+    return t < 32 ? 32 / t : 1;
+}
+
 int launch_row(tacaw_ctx* ctx, int mode, const RowArgs& a, cudaStream_t st) {
     if (a.nwaves <= 0) return TACAW_OK;
     switch (ctx->grid.nx) {
@@ -294,12 +389,13 @@ template <int N>
 struct ColCfg {
     using P = Plan2<N>;
     static constexpr int E = P::E, T = P::T;
-    static constexpr int WC = (N >= 2048) ? 4 : 8;          // adjacent columns transformed together
+    static constexpr int WC = (N >= 1024) ? 4 : 8;          // adjacent columns transformed together
+    static constexpr bool PY_SMEM = (N <= 512);              // Py table in shared memory (else read through L1)
     static constexpr int THREADS = T * WC;
     static constexpr int XE = exch2_elems(N, WC);
-    static constexpr int MINB = (N <= 512) ? 3 : (N == 1024 ? 2 : 1);
+    static constexpr int MINB = (N <= 1024) ? 3 : 1;
     // twiddles | Py | staging tile [N][WC] | exchange
-    static constexpr size_t smem() { return sizeof(float2) * ((size_t)P::TW_ELEMS + N + (size_t)N * WC + XE); }
+    static constexpr size_t smem() { return sizeof(float2) * ((size_t)P::TW_ELEMS + (PY_SMEM ? N : 0) + (size_t)N * WC + XE); }
 };
 
 // Work items of a column launch are (column group, wave) pairs, flattened as gi*nwaves + w over the
@@ -317,15 +413,14 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MINB) k_col(Col
     const int lt = threadIdx.x;
     const int c = lt % WC, tid = lt / WC;
     float2* tw = smem;
-    float2* sPy = smem + P::TW_ELEMS;             // Py[ky] * pscale
-    float2* sS = sPy + N;                         // staging tile
+    float2* sPy = smem + P::TW_ELEMS;             // Py[ky]
+    float2* sS = sPy + (C::PY_SMEM ? N : 0);      // staging tile
     float2* ex = sS + N * WC;
+    pdl_launch_dependents();
     fft2_load_twiddles<N>(tw, a.roots, lt, C::THREADS);
-    if constexpr (MODE != COL_INV) {
-        for (int i = lt; i < N; i += C::THREADS) {
-            const float2 p = a.py[i];
-            sPy[i] = make_float2(p.x * a.pscale, p.y * a.pscale);
-        }
+    if constexpr (MODE != COL_INV && C::PY_SMEM) {
+        for (int i = lt; i < N / 2; i += C::THREADS) cp_async16(sPy + 2 * i, a.py + 2 * i);
+        cp_async_commit();
     }
     const float2* twp = tw + tid;
     const int NG = a.nx / WC;
@@ -351,6 +446,7 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MINB) k_col(Col
 
     auto body = [&](auto sync) {
         int gi = 0, w = 0;
+        pdl_wait();                              // the tables above do not depend on the previous kernel; the waves do
         if (i0 < i1) {
             gi = (int)(i0 / a.nwaves);
             w = (int)(i0 - (long long)gi * a.nwaves);
@@ -375,6 +471,7 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MINB) k_col(Col
                     const int km = a.kmax[ix];
                     live = km >= 0;
                     px = a.px[ix];
+                    px = make_float2(px.x * a.pscale, px.y * a.pscale);
                     dlo = km - tid;
                     dhi = km + tid;
                 }
@@ -397,7 +494,7 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MINB) k_col(Col
                         x[m] = make_float2(0.f, 0.f);
                     } else {
                         const bool keep = (T * m < N / 2) ? (T * m <= dlo) : (N - T * m <= dhi);
-                        const float2 p = cmul(px, sPy[tid + T * m]);
+                        const float2 p = cmul(px, C::PY_SMEM ? sPy[tid + T * m] : __ldg(a.py + tid + T * m));
                         x[m] = keep ? cmul(x[m], p) : make_float2(0.f, 0.f);
                     }
                 }
@@ -457,7 +554,7 @@ static int launch_col_nb(tacaw_ctx* ctx, const ColArgs& a0, cudaStream_t st) {
     if (ctas > a.nitems) ctas = a.nitems;
     a.ipc = (int)((a.nitems + ctas - 1) / ctas);
     ctas = (a.nitems + a.ipc - 1) / a.ipc;
-    kern<<<(unsigned)ctas, C::THREADS, smem, st>>>(a);
+    TACAW_CUDA(ctx, launch_pdl(kern, (unsigned)ctas, C::THREADS, smem, st, a.pdl != 0, a));
     ctx->launches++;
     if (MODE == COL_LASTQ && !all) {
         const int c0 = nlo * C::WC, c1 = (NG - nhi) * C::WC;
