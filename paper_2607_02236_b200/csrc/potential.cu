@@ -250,7 +250,8 @@ int launch_potential(tacaw_ctx* ctx, const double* d_pos, const int32_t* d_speci
     int* offsets = counts + nkeys;
     TACAW_CUDA(ctx, cudaMemsetAsync(counts, 0, sizeof(int) * (2 * (size_t)nkeys + 1), st));
     TACAW_CUDA(ctx, cudaMemsetAsync(d_nclamped, 0, 2 * sizeof(int), st));
-    TACAW_CUDA(ctx, cudaMemsetAsync(d_V, 0, sizeof(float2) * (size_t)nframes * nslices * nx * ny, st));
+    // d_V is not cleared: k_potential writes every in-band (h,k), and the column pass that follows reads only those
+    if (ntotal == 0) TACAW_CUDA(ctx, cudaMemsetAsync(d_V, 0, sizeof(float2) * (size_t)nframes * nslices * nx * ny, st));
     if (ntotal > 0) {
         k_atom_keys<<<(unsigned)((ntotal + 255) / 256), 256, 0, st>>>(d_pos, d_species, natoms, ntotal, nspecies, dz, nslices,
                                                                      z0, 1.0 / ctx->grid.lx_A, 1.0 / ctx->grid.ly_A, keys, ux,

@@ -465,22 +465,26 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MINB) k_col(Col
                 cur_gi = gi;
                 const int ix = group_of(gi) * WC + c;
                 coloff = (size_t)ix + (size_t)tid * a.nx;
+                // a column entirely outside the mask is never written by the row kernel: it is not
+                // used (NaN * 0 would not be 0) and comes out as zeros
+                const int km = a.kmax[ix];
+                live = km >= 0;
+                dlo = km - tid;
+                dhi = km + tid;
                 if constexpr (MODE != COL_INV) {
-                    // a column entirely outside the mask is never written by the row kernel: it is not
-                    // used (NaN * 0 would not be 0) and comes out as zeros
-                    const int km = a.kmax[ix];
-                    live = km >= 0;
                     px = a.px[ix];
                     px = make_float2(px.x * a.pscale, px.y * a.pscale);
-                    dlo = km - tid;
-                    dhi = km + tid;
                 }
             }
             float2* wc = a.waves + (size_t)w * npix + coloff;
             const size_t rs = (size_t)T * a.nx;
             float2 x[E];
 #pragma unroll
-            for (int m = 0; m < E; ++m) x[m] = live ? sS[(tid + T * m) * WC + c] : make_float2(0.f, 0.f);
+            for (int m = 0; m < E; ++m) {
+                // COL_INV input (V(q) or the probe aperture): only |k| <= kmax[ix] was written
+                const bool keep = (MODE != COL_INV) || ((T * m < N / 2) ? (T * m <= dlo) : (N - T * m <= dhi));
+                x[m] = (live && keep) ? sS[(tid + T * m) * WC + c] : make_float2(0.f, 0.f);
+            }
             int wn = w + 1, gn = gi;
             if (wn == a.nwaves) { wn = 0; ++gn; }
             const bool more = (i + 1 < i1);
