@@ -294,6 +294,23 @@ def main():
         e2e = {"value": wl.slice_steps * nrep * world / (e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                "d2h_bytes_per_step": int(d2h), "steps": nrep}
 
+    # Welch average over half-length chunks (nu = 2) of the resident time-ordered buffer
+    welch = None
+    if wl.nframes >= 16:
+        Lc = 1 << ((wl.nframes // 2).bit_length() - 1)
+        r.spectrum_welch(Lc, 2)
+        w0, w1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        w0.record()
+        for _ in range(5):
+            _, _, nch = r.spectrum_welch(Lc, 2)
+        w1.record()
+        torch.cuda.synchronize()
+        w_ms = w0.elapsed_time(w1) / 5
+        in_bytes = nch * Lc * wl.nprobes * int(r.roi.numel()) * 8
+        welch = {"chunk_len": Lc, "chunk_overlap": 2, "nchunks": int(nch), "window": "hann", "ms": w_ms,
+                 "spectra_per_s": wl.nprobes * int(r.roi.numel()) / (w_ms * 1e-3), "read_GBps": in_bytes / (w_ms * 1e-3) / 1e9}
+
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         v, dt, cores = oracle_sample(wl, max(1, args.ref_frames))
@@ -308,7 +325,7 @@ def main():
                 "config": workload_config(wl, {"roi_pixels": int(r.roi.numel()), "frames_per_block": r.fpb,
                                                "parallelism": f"replicas x{world} (independent scan batches, no collective)"}),
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
-                "spectra_per_s": wl.nprobes * int(r.roi.numel()) * args.steps * world / (elapsed_ms * 1e-3)}
+                "spectra_per_s": wl.nprobes * int(r.roi.numel()) * args.steps * world / (elapsed_ms * 1e-3), "welch": welch}
         print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()

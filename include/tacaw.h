@@ -63,6 +63,10 @@ typedef struct {
 
 #define TACAW_WINDOW_RECT 0
 #define TACAW_WINDOW_HANN 1  /* periodic Hann, w_f = 1/2 - 1/2 cos(2 pi f/T) (:142, :182; reading G9) */
+/* further windows of tacaw_make_window (Appendix A), all in the periodic form x = f/n */
+#define TACAW_WINDOW_TUKEY 2            /* param = alpha in [0,1]: cosine tapers of total fractional width alpha; 1 = Hann, 0 = rect (:170) */
+#define TACAW_WINDOW_BLACKMAN_HARRIS 3  /* 4-term, 0.35875 - 0.48829 cos(2 pi x) + 0.14128 cos(4 pi x) - 0.01168 cos(6 pi x) */
+#define TACAW_WINDOW_KAISER 4           /* param = beta >= 0: I0(beta sqrt(1 - (2x-1)^2)) / I0(beta) */
 
 /* Library version string and the SM architecture it was compiled for ("sm_100a"). */
 const char *tacaw_version(void);
@@ -143,6 +147,24 @@ int tacaw_accumulate(tacaw_ctx *ctx, const void *d_qwaves, int nwaves, const int
 int tacaw_spectrum(tacaw_ctx *ctx, const void *d_buf, int nprobes, int64_t nroi, int nframes, double dt_fs,
                    int window, double temperature_K, double emin_meV, double emax_meV, float *d_I,
                    double *E_axis_meV_out, int *nE, void *stream);
+
+/* Window table, HOST, fp64 (PAPER.md:142 "multiplied by a window function before the Fourier transform", :170-182):
+ * w_out[f], f = 0..n-1, for kind = TACAW_WINDOW_*; param as listed with the kinds.  Returns TACAW_E_ARG on a bad
+ * kind or parameter. */
+int tacaw_make_window(int kind, int n, double param, double *w_out);
+
+/* Welch method over trajectory chunks (Eq.(2) :126):
+ * the time-ordered buffer holds nframes_total frames; chunk n covers frames s_n .. s_n + L - 1 with
+ * s_0 = 0, s_{n+1} = s_n + L/nu (remainder-less division), for every n with s_n + L <= nframes_total (N chunks);
+ *   I[p][e][r] = (1/N) sum_n B(E_e/(k_B T_K)) |Phi_n|^2 / (L sum_f w_f^2),  Phi_n = DFT over the chunk of w_f buf
+ * with E_k = h k'/(L dt).  L = chunk_len: power of two in [8, 2048]; nu = chunk_overlap >= 1.
+ * window_table HOST double [L] (tacaw_make_window or the caller's own).  N = 0 (buffer shorter than a chunk)
+ * leaves d_I untouched.  nchunks HOST out (may be NULL).  Other arguments as tacaw_spectrum;
+ * d_buf DEVICE complex64 [nprobes][nframes_total][nroi], d_I DEVICE float [nprobes][nE][nroi]. */
+int tacaw_spectrum_welch(tacaw_ctx *ctx, const void *d_buf, int nprobes, int64_t nroi, int nframes_total, int chunk_len,
+                         int chunk_overlap, double dt_fs, const double *window_table, double temperature_K,
+                         double emin_meV, double emax_meV, float *d_I, double *E_axis_meV_out, int *nE, int *nchunks,
+                         void *stream);
 
 /* Convenience for host-resident data (bench.py's end-to-end leg): same as the calls above but the
  * named buffers are HOST memory; the library stages them through its own device scratch with

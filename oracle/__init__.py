@@ -2,8 +2,9 @@
 
 Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
 this package.  It never imports paper_2607_02236_b200's CUDA binding and shares no code with it.
-Every function is a marshalling shim around the C routine of the same name; the arithmetic and the
-paper citations live in the C file's header.
+Functions up to `spectrum` are marshalling shims around the C routine of the same name; the arithmetic and
+the paper citations live in the C file's header.  The Welch / window additions at the end are
+plain numpy on top of oracle_spectrum_table, each citing the passage it follows.
 """
 from __future__ import annotations
 
@@ -208,3 +209,77 @@ def spectrum(buf: np.ndarray, dt_fs: float, window_kind: int, temperature_K: flo
         raise RuntimeError(f"oracle_spectrum failed: {rc}")
     assert nE.value == E.size
     return I, Eo
+
+
+# ---------------------------------------------------------------------------------------------
+# Welch chunks with Eq.(2) averaging, further window functions.
+
+def window_table(kind: str, n: int, param: float = 0.0) -> np.ndarray:
+    """Window functions of PAPER.md:170-182 / Appendix A in the periodic form x = f/n (reading G9: the periodic Hann is
+    the variant for which the zero-loss peak does not leak, :182).  'tukey': param = alpha, the summed fractional width of
+    the two cosine tapers; alpha = 1 is Hann, alpha = 0 is rectangular (:170).  'blackman_harris': 4-term cosine sum.
+    'kaiser': param = beta, I0(beta sqrt(1 - (2x-1)^2))/I0(beta) (numpy.i0 is the library Bessel routine)."""
+    x = np.arange(n, dtype=np.float64) / n
+    if kind == "rect":
+        return np.ones(n)
+    if kind == "hann":
+        return 0.5 - 0.5 * np.cos(2 * np.pi * x)
+    if kind == "tukey":
+        a = float(param)
+        if a == 0.0:
+            return np.ones(n)
+        w = np.ones(n)
+        up = x < a / 2
+        dn = x > 1 - a / 2
+        w[up] = 0.5 * (1 - np.cos(2 * np.pi * x[up] / a))
+        w[dn] = 0.5 * (1 - np.cos(2 * np.pi * (1 - x[dn]) / a))
+        return w
+    if kind == "blackman_harris":
+        return 0.35875 - 0.48829 * np.cos(2 * np.pi * x) + 0.14128 * np.cos(4 * np.pi * x) - 0.01168 * np.cos(6 * np.pi * x)
+    if kind == "kaiser":
+        u = 2 * x - 1
+        return np.i0(param * np.sqrt(np.maximum(0.0, 1 - u * u))) / np.i0(param)
+    raise ValueError(kind)
+
+
+def chunk_starts(nframes_total: int, chunk_len: int, chunk_overlap: int):
+    """'If a chunk indexed by n starts at snapshot s_n, then the next chunk starts at
+    s_{n+1} = s_n + L/nu, using remainder-less division'; only complete chunks are used."""
+    step = chunk_len // chunk_overlap
+    out, s = [], 0
+    while s + chunk_len <= nframes_total:
+        out.append(s)
+        s += step
+    return out
+
+
+def spectrum_table(buf: np.ndarray, frame0: int, nframes: int, dt_fs: float, w: np.ndarray, temperature_K: float,
+                   emin: float = -np.inf, emax: float = np.inf) -> Tuple[np.ndarray, np.ndarray]:
+    """O9 on frames [frame0, frame0+nframes) of buf [P][Ttot][Q] with the window table w[nframes]."""
+    buf = np.ascontiguousarray(buf, dtype=np.complex128)
+    w = np.ascontiguousarray(w, dtype=np.float64)
+    P, Ttot, Q = buf.shape
+    E, _ = energy_axis(nframes, dt_fs, emin, emax)
+    I = np.empty((P, E.size, Q), dtype=np.float64)
+    Eo = np.empty(E.size, dtype=np.float64)
+    nE = C.c_int(0)
+    rc = lib().oracle_spectrum_table(_p(buf), C.c_int(P), C.c_int64(Q), C.c_int(Ttot), C.c_int(frame0), C.c_int(nframes),
+                                     C.c_double(dt_fs), _p(w), C.c_double(temperature_K), C.c_double(emin), C.c_double(emax),
+                                     _p(I), _p(Eo), C.byref(nE))
+    if rc != 0:
+        raise RuntimeError(f"oracle_spectrum_table failed: {rc}")
+    return I, Eo
+
+
+def spectrum_welch(buf: np.ndarray, chunk_len: int, chunk_overlap: int, dt_fs: float, w: np.ndarray, temperature_K: float,
+                   emin: float = -np.inf, emax: float = np.inf):
+    """Eq.(2): the average over the N trajectory chunks of I_i(q,E), each chunk windowed, transformed,
+    squared and Bose-corrected as in O9 (:142).  Returns (I [P][nE][Q], E [nE], N)."""
+    starts = chunk_starts(buf.shape[1], chunk_len, chunk_overlap)
+    acc, E = None, None
+    for s in starts:
+        I, E = spectrum_table(buf, s, chunk_len, dt_fs, w, temperature_K, emin, emax)
+        acc = I / len(starts) if acc is None else acc + I / len(starts)
+    if E is None:
+        E, _ = energy_axis(chunk_len, dt_fs, emin, emax)
+    return acc, E, len(starts)

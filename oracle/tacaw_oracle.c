@@ -438,9 +438,11 @@ int oracle_energy_axis(int nframes, double dt_fs, double emin, double emax, doub
     return c;
 }
 
-/* O9.  buf [nprobes][nframes][nroi] complex -> I [nprobes][nE][nroi] (double).  E_out [nE]. */
-int oracle_spectrum(const double *buf, int nprobes, int64_t nroi, int nframes, double dt_fs, int window,
-                    double temperature_K, double emin, double emax, double *I, double *E_out, int *nE_out) {
+/* O9 with the window given as a table w[nframes], on frames
+ * [frame0, frame0 + nframes) of a buffer [nprobes][nframes_total][nroi]; I [nprobes][nE][nroi] (double), E_out [nE]. */
+int oracle_spectrum_table(const double *buf, int nprobes, int64_t nroi, int nframes_total, int frame0, int nframes, double dt_fs,
+                          const double *w, double temperature_K, double emin, double emax, double *I, double *E_out,
+                          int *nE_out) {
     const double kb_mev = 8.617333262e-5 * 1e3;
     int nE = oracle_energy_axis(nframes, dt_fs, emin, emax, NULL, NULL);
     if (nE_out) *nE_out = nE;
@@ -449,8 +451,6 @@ int oracle_spectrum(const double *buf, int nprobes, int64_t nroi, int nframes, d
     int32_t *bins = (int32_t *)malloc(sizeof(int32_t) * (size_t)(nE > 0 ? nE : 1));
     oracle_energy_axis(nframes, dt_fs, emin, emax, E, bins);
     if (E_out) memcpy(E_out, E, sizeof(double) * (size_t)nE);
-    double *w = (double *)malloc(sizeof(double) * (size_t)nframes);
-    oracle_window(window, nframes, w);
     double sw2 = 0.0;
     for (int f = 0; f < nframes; ++f) sw2 += w[f] * w[f];
     double norm = 1.0 / ((double)nframes * sw2);
@@ -462,7 +462,7 @@ int oracle_spectrum(const double *buf, int nprobes, int64_t nroi, int nframes, d
         for (int64_t s = 0; s < nser; ++s) {
             int64_t p = s / nroi, r = s % nroi;
             for (int f = 0; f < nframes; ++f) {
-                const double *src = buf + 2 * ((p * nframes + f) * nroi + r);
+                const double *src = buf + 2 * ((p * nframes_total + frame0 + f) * nroi + r);
                 x[2 * f] = w[f] * src[0];
                 x[2 * f + 1] = w[f] * src[1];
             }
@@ -474,6 +474,16 @@ int oracle_spectrum(const double *buf, int nprobes, int64_t nroi, int nframes, d
         }
         free(x);
     }
-    free(E); free(bins); free(w);
+    free(E); free(bins);
     return 0;
+}
+
+/* O9.  buf [nprobes][nframes][nroi] complex -> I [nprobes][nE][nroi] (double).  E_out [nE].  window: O10. */
+int oracle_spectrum(const double *buf, int nprobes, int64_t nroi, int nframes, double dt_fs, int window,
+                    double temperature_K, double emin, double emax, double *I, double *E_out, int *nE_out) {
+    double *w = (double *)malloc(sizeof(double) * (size_t)nframes);
+    oracle_window(window, nframes, w);
+    int rc = oracle_spectrum_table(buf, nprobes, nroi, nframes, 0, nframes, dt_fs, w, temperature_K, emin, emax, I, E_out, nE_out);
+    free(w);
+    return rc;
 }

@@ -17,7 +17,9 @@ LIB_PATH = os.path.join(_HERE, "libtacaw.so")
 
 EXPORTS = ["tacaw_version", "tacaw_create", "tacaw_destroy", "tacaw_last_error", "tacaw_launch_count",
            "tacaw_build_slices", "tacaw_build_slices_host", "tacaw_make_probes", "tacaw_propagate",
-           "tacaw_make_roi", "tacaw_accumulate", "tacaw_spectrum"]
+           "tacaw_make_roi", "tacaw_accumulate", "tacaw_spectrum", "tacaw_make_window", "tacaw_spectrum_welch"]
+
+WINDOWS = {"rect": 0, "hann": 1, "tukey": 2, "blackman_harris": 3, "kaiser": 4}
 
 ROI_MODES = {"full": 0, "disc": 1, "annulus": 2, "rect": 3}
 
@@ -246,3 +248,36 @@ class Tacaw:
                                      self._stream())
         self._check(rc, "tacaw_spectrum")
         return out, E[: nE.value].copy()
+
+    def spectrum_welch(self, buf, chunk_len: int, chunk_overlap: int, dt_fs: float, window_table, temperature_K: float,
+                       emin: float = -np.inf, emax: float = np.inf, out=None):
+        """tacaw_spectrum_welch: returns (I float32 CUDA [P][nE][Q] averaged over the chunks, E float64 numpy [nE], nchunks)."""
+        torch = self.torch
+        P, Ttot, Q = buf.shape
+        w = np.ascontiguousarray(window_table, dtype=np.float64)
+        if w.shape != (chunk_len,):
+            raise ValueError("window_table must have chunk_len entries")
+        nE, nch = C.c_int(0), C.c_int(0)
+        E = np.empty(chunk_len, dtype=np.float64)
+        args = [C.c_int(P), C.c_int64(Q), C.c_int(Ttot), C.c_int(chunk_len), C.c_int(chunk_overlap), C.c_double(dt_fs),
+                w.ctypes.data_as(C.c_void_p), C.c_double(temperature_K), C.c_double(emin), C.c_double(emax)]
+        rc = self.lib.tacaw_spectrum_welch(self._ctx, None, *args, None, E.ctypes.data_as(C.c_void_p), C.byref(nE), C.byref(nch),
+                                           self._stream())
+        self._check(rc, "tacaw_spectrum_welch")
+        if out is None:
+            out = torch.zeros((P, nE.value, Q), dtype=torch.float32, device=buf.device)
+        rc = self.lib.tacaw_spectrum_welch(self._ctx, self._dev(buf, torch.complex64, "buf"), *args,
+                                           self._dev(out, torch.float32, "I"), E.ctypes.data_as(C.c_void_p), C.byref(nE),
+                                           C.byref(nch), self._stream())
+        self._check(rc, "tacaw_spectrum_welch")
+        return out, E[: nE.value].copy(), nch.value
+
+
+def make_window(kind: str, n: int, param: float = 0.0) -> np.ndarray:
+    """tacaw_make_window (host): fp64 table of a periodic window ('rect', 'hann', 'tukey', 'blackman_harris', 'kaiser')."""
+    lib = load_library()
+    w = np.empty(n, dtype=np.float64)
+    rc = lib.tacaw_make_window(C.c_int(WINDOWS[kind]), C.c_int(n), C.c_double(param), w.ctypes.data_as(C.c_void_p))
+    if rc != 0:
+        raise TacawError(f"tacaw_make_window failed ({rc})")
+    return w

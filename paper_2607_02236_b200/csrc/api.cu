@@ -525,20 +525,18 @@ int tacaw_accumulate(tacaw_ctx* ctx, const void* d_qwaves, int nwaves, const int
                          nframes, st);
 }
 
-int tacaw_spectrum(tacaw_ctx* ctx, const void* d_buf, int nprobes, int64_t nroi, int nframes, double dt_fs, int window,
-                   double temperature_K, double emin, double emax, float* d_I, double* E_out, int* nE_out, void* stream) {
-    if (!ctx) return TACAW_E_ARG;
-    if (nprobes < 0 || nroi < 0 || nframes <= 0 || !(dt_fs > 0) || !(temperature_K > 0) || !nE_out ||
-        (window != TACAW_WINDOW_RECT && window != TACAW_WINDOW_HANN))
-        return fail(ctx, TACAW_E_ARG, "tacaw_spectrum: bad argument");
-    if (nframes < 8 || nframes > 2048 || (nframes & (nframes - 1))) return fail(ctx, TACAW_E_UNSUPPORTED, "nframes must be a power of two in [8, 2048]");
+// Shared core of tacaw_spectrum / tacaw_spectrum_welch: chunks of L frames starting every `step` frames of a
+// [nprobes][nframes_total][nroi] buffer, window table w[L] (fp64, host), I = (1/nchunks) sum_i I_i.
+static int spectrum_core(tacaw_ctx* ctx, const void* d_buf, int nprobes, int64_t nroi, int nframes_total, int L, int step,
+                         int nchunks, double dt_fs, const double* w, double temperature_K, double emin, double emax, float* d_I,
+                         double* E_out, int* nE_out, cudaStream_t st, const char* who) {
+    if (L < 8 || L > 2048 || (L & (L - 1))) return fail(ctx, TACAW_E_UNSUPPORTED, std::string(who) + ": the transform length must be a power of two in [8, 2048]");
     const double h_mev_fs = 4135.667696, kb_mev = 8.617333262e-2;
-    const int T = nframes;
-    // ascending axis k' = -T/2 .. T/2-1; keep [emin, emax] with 1e-9 meV slack (reading G11)
+    // ascending axis k' = -L/2 .. L/2-1; keep [emin, emax] with 1e-9 meV slack (reading G11)
     int e_lo = -1, nE = 0;
     std::vector<double> E;
-    for (int i = 0; i < T; ++i) {
-        double e = h_mev_fs * (double)(i - T / 2) / ((double)T * dt_fs);
+    for (int i = 0; i < L; ++i) {
+        double e = h_mev_fs * (double)(i - L / 2) / ((double)L * dt_fs);
         if (e < emin - 1e-9 || e > emax + 1e-9) continue;
         if (e_lo < 0) e_lo = i;
         E.push_back(e);
@@ -546,34 +544,107 @@ int tacaw_spectrum(tacaw_ctx* ctx, const void* d_buf, int nprobes, int64_t nroi,
     }
     *nE_out = nE;
     if (E_out) for (int i = 0; i < nE; ++i) E_out[i] = E[i];
-    if (!d_I || nE == 0 || nprobes == 0 || nroi == 0) return TACAW_OK;
-    if (!d_buf) return fail(ctx, TACAW_E_ARG, "tacaw_spectrum: null buffer");
-    cudaStream_t st = (cudaStream_t)stream;
-    std::vector<float> tab(2 * (size_t)T + (size_t)T + (size_t)nE);   // roots (float2 x T), window, bose
+    if (!d_I || nE == 0 || nprobes == 0 || nroi == 0 || nchunks == 0) return TACAW_OK;
+    if (!d_buf) return fail(ctx, TACAW_E_ARG, std::string(who) + ": null buffer");
+    std::vector<float> tab(2 * (size_t)L + (size_t)L + (size_t)nE);   // roots (float2 x L), window, bose
     double sw2 = 0.0;
-    std::vector<double> w(T);
-    for (int f = 0; f < T; ++f) {
-        w[f] = (window == TACAW_WINDOW_HANN) ? 0.5 - 0.5 * std::cos(2.0 * M_PI * (double)f / (double)T) : 1.0;
-        sw2 += w[f] * w[f];
-    }
-    for (int j = 0; j < T; ++j) {
-        double ang = -2.0 * M_PI * (double)j / (double)T;
+    for (int f = 0; f < L; ++f) sw2 += w[f] * w[f];
+    if (!(sw2 > 0)) return fail(ctx, TACAW_E_ARG, std::string(who) + ": window is identically zero");
+    for (int j = 0; j < L; ++j) {
+        double ang = -2.0 * M_PI * (double)j / (double)L;
         tab[2 * j] = (float)std::cos(ang);
         tab[2 * j + 1] = (float)std::sin(ang);
-        tab[2 * (size_t)T + j] = (float)w[j];
+        tab[2 * (size_t)L + j] = (float)w[j];
     }
     for (int i = 0; i < nE; ++i) {
         double x = E[i] / (kb_mev * temperature_K);
         double B = (x == 0.0) ? 1.0 : x / (-std::expm1(-x));
-        tab[3 * (size_t)T + i] = (float)(B / ((double)T * sw2));
+        tab[3 * (size_t)L + i] = (float)(B / ((double)L * sw2 * (double)nchunks));
     }
     int rc = ensure(ctx, (void**)&ctx->d_spec_tab, &ctx->spec_tab_bytes, sizeof(float) * tab.size());
     if (rc) return rc;
     if ((rc = upload(ctx, ctx->d_spec_tab, tab.data(), sizeof(float) * tab.size(), st))) return rc;
-    rc = launch_spectrum(ctx, (const float2*)d_buf, nprobes, nroi, T, (const float2*)ctx->d_spec_tab,
-                         ctx->d_spec_tab + 2 * (size_t)T, ctx->d_spec_tab + 3 * (size_t)T, e_lo, nE, d_I, st);
-    if (rc) return rc;
+    for (int c = 0; c < nchunks; ++c) {
+        rc = launch_spectrum(ctx, (const float2*)d_buf + (size_t)c * step * (size_t)nroi, nprobes, nroi, L,
+                             (size_t)nframes_total * (size_t)nroi, c > 0, (const float2*)ctx->d_spec_tab,
+                             ctx->d_spec_tab + 2 * (size_t)L, ctx->d_spec_tab + 3 * (size_t)L, e_lo, nE, d_I, st);
+        if (rc) return rc;
+    }
     return TACAW_OK;
+}
+
+// modified Bessel function I0 (power series; converges for every beta used as a Kaiser parameter)
+static double bessel_i0(double x) {
+    double sum = 1.0, term = 1.0;
+    const double q = 0.25 * x * x;
+    for (int k = 1; k < 500; ++k) {
+        term *= q / ((double)k * (double)k);
+        sum += term;
+        if (term < 1e-17 * sum) break;
+    }
+    return sum;
+}
+
+int tacaw_make_window(int kind, int n, double param, double* w_out) {
+    if (n <= 0 || !w_out) return TACAW_E_ARG;
+    for (int f = 0; f < n; ++f) {
+        const double x = (double)f / (double)n;          // periodic form: sample f of a window of period n
+        double v = 1.0;
+        switch (kind) {
+            case TACAW_WINDOW_RECT: v = 1.0; break;
+            case TACAW_WINDOW_HANN: v = 0.5 - 0.5 * std::cos(2.0 * M_PI * x); break;
+            case TACAW_WINDOW_TUKEY: {
+                const double a = param;
+                if (!(a >= 0.0 && a <= 1.0)) return TACAW_E_ARG;
+                if (a == 0.0) v = 1.0;
+                else if (x < 0.5 * a) v = 0.5 * (1.0 - std::cos(2.0 * M_PI * x / a));
+                else if (x <= 1.0 - 0.5 * a) v = 1.0;
+                else v = 0.5 * (1.0 - std::cos(2.0 * M_PI * (1.0 - x) / a));
+                break;
+            }
+            case TACAW_WINDOW_BLACKMAN_HARRIS:
+                v = 0.35875 - 0.48829 * std::cos(2.0 * M_PI * x) + 0.14128 * std::cos(4.0 * M_PI * x) - 0.01168 * std::cos(6.0 * M_PI * x);
+                break;
+            case TACAW_WINDOW_KAISER: {
+                if (!(param >= 0.0)) return TACAW_E_ARG;
+                const double u = 2.0 * x - 1.0;
+                v = bessel_i0(param * std::sqrt(std::fmax(0.0, 1.0 - u * u))) / bessel_i0(param);
+                break;
+            }
+            default: return TACAW_E_ARG;
+        }
+        w_out[f] = v;
+    }
+    return TACAW_OK;
+}
+
+int tacaw_spectrum(tacaw_ctx* ctx, const void* d_buf, int nprobes, int64_t nroi, int nframes, double dt_fs, int window,
+                   double temperature_K, double emin, double emax, float* d_I, double* E_out, int* nE_out, void* stream) {
+    if (!ctx) return TACAW_E_ARG;
+    if (nprobes < 0 || nroi < 0 || nframes <= 0 || !(dt_fs > 0) || !(temperature_K > 0) || !nE_out ||
+        (window != TACAW_WINDOW_RECT && window != TACAW_WINDOW_HANN))
+        return fail(ctx, TACAW_E_ARG, "tacaw_spectrum: bad argument");
+    if (nframes < 8 || nframes > 2048 || (nframes & (nframes - 1))) return fail(ctx, TACAW_E_UNSUPPORTED, "nframes must be a power of two in [8, 2048]");
+    std::vector<double> w(nframes);
+    tacaw_make_window(window, nframes, 0.0, w.data());
+    return spectrum_core(ctx, d_buf, nprobes, nroi, nframes, nframes, nframes, 1, dt_fs, w.data(), temperature_K, emin, emax, d_I,
+                         E_out, nE_out, (cudaStream_t)stream, "tacaw_spectrum");
+}
+
+int tacaw_spectrum_welch(tacaw_ctx* ctx, const void* d_buf, int nprobes, int64_t nroi, int nframes_total, int chunk_len,
+                         int chunk_overlap, double dt_fs, const double* window_table, double temperature_K, double emin,
+                         double emax, float* d_I, double* E_out, int* nE_out, int* nchunks_out, void* stream) {
+    if (!ctx) return TACAW_E_ARG;
+    if (nprobes < 0 || nroi < 0 || nframes_total <= 0 || chunk_len <= 0 || chunk_overlap <= 0 || !(dt_fs > 0) ||
+        !(temperature_K > 0) || !nE_out || !window_table)
+        return fail(ctx, TACAW_E_ARG, "tacaw_spectrum_welch: bad argument");
+    const int step = chunk_len / chunk_overlap;        // s_{n+1} = s_n + L/nu, remainder-less division
+    if (step <= 0) return fail(ctx, TACAW_E_ARG, "tacaw_spectrum_welch: chunk_overlap exceeds chunk_len");
+    int nchunks = 0;
+    for (int s0 = 0; s0 + chunk_len <= nframes_total; s0 += step) ++nchunks;
+    if (nchunks_out) *nchunks_out = nchunks;
+    return spectrum_core(ctx, d_buf, nprobes, nroi, nframes_total, chunk_len, step, nchunks, dt_fs, window_table, temperature_K,
+                         emin, emax, d_I, E_out, nE_out, (cudaStream_t)stream, "tacaw_spectrum_welch");
 }
 
 }  // extern "C"

@@ -122,7 +122,9 @@ int launch_probe_fill(tacaw_ctx* ctx, const uint32_t* d_uxy /*[P][2] fixed-point
                       const int* d_kap /*[nx]*/, float amp, float2* d_waves, cudaStream_t st);
 int launch_gather(tacaw_ctx* ctx, const float2* d_q, int nwaves, const int* d_wp, const int* d_wf, const int* d_idx,
                   int64_t nroi, float2* d_buf, int nprobes, int nframes, cudaStream_t st);
-int launch_spectrum(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int64_t nroi, int nframes, const float2* d_roots,
+// probe_stride: elements between the series blocks of consecutive probes; accumulate: add to d_I instead of storing
+int launch_spectrum(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int64_t nroi, int nframes, size_t probe_stride,
+                    int accumulate, const float2* d_roots,
                     const float* d_window, const float* d_bose, int e_lo, int nE, float* d_I, cudaStream_t st);
 
 }  // namespace tacaw

@@ -22,6 +22,7 @@ struct SpecCfg {
 
 template <int N>
 __global__ void __launch_bounds__(SpecCfg<N>::THREADS) k_spectrum(const float2* __restrict__ buf, long long nroi,
+                                                                  size_t probe_stride, int accumulate,
                                                                   const float2* __restrict__ roots,
                                                                   const float* __restrict__ window,
                                                                   const float* __restrict__ bose, int e_lo, int nE,
@@ -49,7 +50,7 @@ __global__ void __launch_bounds__(SpecCfg<N>::THREADS) k_spectrum(const float2* 
     const int p = blockIdx.y;
     const long long r = (long long)blockIdx.x * WQ + c;
     const bool live = r < nroi;
-    const float2* src = buf + (size_t)p * N * (size_t)nroi + (live ? r : 0);
+    const float2* src = buf + (size_t)p * probe_stride + (live ? r : 0);
     float2 x[E];
 #pragma unroll
     for (int m = 0; m < E; ++m) {
@@ -71,12 +72,17 @@ __global__ void __launch_bounds__(SpecCfg<N>::THREADS) k_spectrum(const float2* 
     for (int m = 0; m < E; ++m) {
         int kbin = tid + T * m;
         int e = ((kbin + N / 2) & (N - 1)) - e_lo;      // position on the ascending energy axis
-        if (e >= 0 && e < nE) dst[(size_t)e * nroi] = bose[e] * (x[m].x * x[m].x + x[m].y * x[m].y);
+        if (e >= 0 && e < nE) {
+            const float v = bose[e] * (x[m].x * x[m].x + x[m].y * x[m].y);
+            // Welch chunks after the first add their share (Eq.(2)); a chunk's launches are stream-ordered
+            dst[(size_t)e * nroi] = accumulate ? dst[(size_t)e * nroi] + v : v;
+        }
     }
 }
 
 template <int N>
-static int launch_spec_n(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int64_t nroi, const float2* roots,
+static int launch_spec_n(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int64_t nroi, size_t probe_stride, int accumulate,
+                         const float2* roots,
                          const float* d_window, const float* d_bose, int e_lo, int nE, float* d_I, cudaStream_t st) {
     using C = SpecCfg<N>;
     size_t smem = (size_t)2 * exch_elems(N, C::WQ) * sizeof(float2) + (C::TWREG ? 0 : (size_t)N * sizeof(float2));
@@ -85,7 +91,7 @@ static int launch_spec_n(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int64
     int64_t gx = (nroi + C::WQ - 1) / C::WQ;
     for (int p0 = 0; p0 < nprobes; p0 += 32768) {
         int np = nprobes - p0 < 32768 ? nprobes - p0 : 32768;
-        kern<<<dim3((unsigned)gx, np), C::THREADS, smem, st>>>(d_buf + (size_t)p0 * N * (size_t)nroi, (long long)nroi, roots,
+        kern<<<dim3((unsigned)gx, np), C::THREADS, smem, st>>>(d_buf + (size_t)p0 * probe_stride, (long long)nroi, probe_stride, accumulate, roots,
                                                               d_window, d_bose, e_lo, nE,
                                                               d_I + (size_t)p0 * nE * (size_t)nroi);
         ctx->launches++;
@@ -94,18 +100,19 @@ static int launch_spec_n(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int64
     return TACAW_OK;
 }
 
-int launch_spectrum(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int64_t nroi, int nframes, const float2* d_roots,
+int launch_spectrum(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int64_t nroi, int nframes, size_t probe_stride,
+                    int accumulate, const float2* d_roots,
                     const float* d_window, const float* d_bose, int e_lo, int nE, float* d_I, cudaStream_t st) {
     switch (nframes) {
-        case 8: return launch_spec_n<8>(ctx, d_buf, nprobes, nroi, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
-        case 16: return launch_spec_n<16>(ctx, d_buf, nprobes, nroi, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
-        case 32: return launch_spec_n<32>(ctx, d_buf, nprobes, nroi, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
-        case 64: return launch_spec_n<64>(ctx, d_buf, nprobes, nroi, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
-        case 128: return launch_spec_n<128>(ctx, d_buf, nprobes, nroi, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
-        case 256: return launch_spec_n<256>(ctx, d_buf, nprobes, nroi, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
-        case 512: return launch_spec_n<512>(ctx, d_buf, nprobes, nroi, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
-        case 1024: return launch_spec_n<1024>(ctx, d_buf, nprobes, nroi, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
-        case 2048: return launch_spec_n<2048>(ctx, d_buf, nprobes, nroi, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+        case 8: return launch_spec_n<8>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+        case 16: return launch_spec_n<16>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+        case 32: return launch_spec_n<32>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+        case 64: return launch_spec_n<64>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+        case 128: return launch_spec_n<128>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+        case 256: return launch_spec_n<256>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+        case 512: return launch_spec_n<512>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+        case 1024: return launch_spec_n<1024>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+        case 2048: return launch_spec_n<2048>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
     }
     return fail(ctx, TACAW_E_UNSUPPORTED, "nframes must be a power of two in [8, 2048]");
 }

@@ -11,7 +11,7 @@ from typing import Dict, List, Optional, Sequence
 
 import numpy as np
 
-from .binding import ROI_MODES, Tacaw, make_roi
+from .binding import ROI_MODES, Tacaw, make_roi, make_window
 
 
 class Runner:
@@ -85,6 +85,13 @@ class Runner:
         wl = self.wl
         emin, emax = wl.e_roi_meV if wl.e_roi_meV is not None else (-np.inf, np.inf)
         return self.tc.spectrum(self.buf, wl.dt_fs, wl.window, wl.temperature_K, emin, emax)
+
+    def spectrum_welch(self, chunk_len: int, chunk_overlap: int = 2, window: str = "hann", param: float = 0.0):
+        """Welch average over trajectory chunks of the time-ordered buffer (Eq.(2)): (I, E, nchunks)."""
+        wl = self.wl
+        emin, emax = wl.e_roi_meV if wl.e_roi_meV is not None else (-np.inf, np.inf)
+        w = make_window(window, chunk_len, param)
+        return self.tc.spectrum_welch(self.buf, chunk_len, chunk_overlap, wl.dt_fs, w, wl.temperature_K, emin, emax)
 
     def run(self) -> Dict[str, object]:
         """Whole path over the workload's frames: returns dict(I, E, roi, buf)."""

@@ -116,6 +116,27 @@ def test_propagate_batch_invariance_and_segments(torch, B, oracle):
     tc.close()
 
 
+@pytest.mark.parametrize("n", [256, 512])
+def test_propagate_wave_tuples_with_odd_frame_runs(torch, B, oracle, n):
+    """The row kernel transforms tuples of waves of one frame (pairs at 256^2 / 512^2); runs of odd length leave a
+    short tuple that repeats its last wave.  Result vs the oracle, and bitwise equal to one wave at a time."""
+    L, lam, dz = 12.0, 0.0370144, 1.4795
+    trans, psi, _ = random_setup(21, n, n, 5, 2, [2])
+    wf = np.array([0, 0, 0, 1, 1], dtype=np.int32)
+    tc = B.Tacaw(n, n, L, L, lam, 9.2e-4, 1)
+    tr_d = [[dev(torch, t, torch.complex64) for t in fr] for fr in trans]
+    full = dev(torch, psi, torch.complex64)
+    tc.propagate(full, wf, tr_d, dz, 1)
+    ref = oracle.propagate(L, L, lam, 1, psi, wf, trans, dz, 1)
+    got = full.cpu().numpy()
+    for i in range(5):
+        assert rel_l2(got[i], ref[i]) <= 2e-5
+        one = dev(torch, psi[i:i + 1], torch.complex64)
+        tc.propagate(one, wf[i:i + 1], tr_d, dz, 1)
+        assert torch.equal(one[0], full[i])
+    tc.close()
+
+
 def test_propagate_l2_grouping_is_transparent(torch, B, monkeypatch):
     n, L, lam, dz = 128, 9.0, 0.0370144, 1.4795
     trans, psi, wf = random_setup(11, n, n, 9, 4, [3])
