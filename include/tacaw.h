@@ -166,6 +166,24 @@ int tacaw_spectrum_welch(tacaw_ctx *ctx, const void *d_buf, int nprobes, int64_t
                          double emin_meV, double emax_meV, float *d_I, double *E_axis_meV_out, int *nE, int *nchunks,
                          void *stream);
 
+/* DetectorSet (PAPER.md:114 "circular and annular -- with arbitrary center and radii -- and custom", :148-150, :257;
+ * SURVEY.md 8(f) item 2).  Two calls:
+ * tacaw_make_detector, HOST, exact: weights_out[r] = 1 if ROI pixel r lies on the detector, else 0, decided in fp64 as
+ *   tx = lambda h/lx - center_rad[0], ty = lambda k/ly - center_rad[1], t2 = tx*tx + ty*ty,
+ *   circular: t2 <= radii_rad[1]^2;  annular: radii_rad[0]^2 <= t2 <= radii_rad[1]^2   (both edges inclusive)
+ *   with (h,k) the signed frequency indices of the native flat index roi_idx[r] (tacaw_make_roi's convention).
+ * tacaw_detect, DEVICE: out[d][e][p] = sum_r weights[d][r] * I[p][e][r]  -- the energy-filtered STEM signal of
+ *   detector d ("Axes of these arrays are [energy, scan-x, scan-y]", :150; p = scan position).  weights may be any
+ *   caller-supplied array (the paper's "custom" detector).
+ * d_I DEVICE float [nprobes][nE][nroi]; d_weights DEVICE float [ndet][nroi]; d_out DEVICE float [ndet][nE][nprobes].
+ * ndet in [1, 8] per call. */
+#define TACAW_DETECTOR_CIRCULAR 0
+#define TACAW_DETECTOR_ANNULAR 1
+int tacaw_make_detector(const tacaw_grid *grid, double lambda_A, int kind, const double *center_rad, const double *radii_rad,
+                        const int32_t *roi_idx, int64_t nroi, float *weights_out);
+int tacaw_detect(tacaw_ctx *ctx, const float *d_I, int nprobes, int nE, int64_t nroi, const float *d_weights, int ndet,
+                 float *d_out, void *stream);
+
 /* Convenience for host-resident data (bench.py's end-to-end leg): same as the calls above but the
  * named buffers are HOST memory; the library stages them through its own device scratch with
  * cudaMemcpyAsync on `stream` and synchronises before returning. */

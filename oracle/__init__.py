@@ -283,3 +283,29 @@ def spectrum_welch(buf: np.ndarray, chunk_len: int, chunk_overlap: int, dt_fs: f
     if E is None:
         E, _ = energy_axis(chunk_len, dt_fs, emin, emax)
     return acc, E, len(starts)
+
+
+# DetectorSet.
+
+def detector_weights(nx: int, ny: int, lx: float, ly: float, lam: float, kind: str, center_rad, radii_rad,
+                     roi_idx: np.ndarray) -> np.ndarray:
+    """'circular and annular -- with arbitrary center and radii' (:114): pixel (h,k) of the ROI is on the detector iff
+    its scattering angle theta = lambda q, measured from the detector centre, lies inside the (inclusive) radii."""
+    idx = np.asarray(roi_idx, dtype=np.int64)
+    ix, iy = idx % nx, idx // nx
+    h = np.where(ix < nx // 2, ix, ix - nx).astype(np.float64)
+    k = np.where(iy < ny // 2, iy, iy - ny).astype(np.float64)
+    tx = lam * h / lx - center_rad[0]
+    ty = lam * k / ly - center_rad[1]
+    t2 = tx * tx + ty * ty
+    on = t2 <= radii_rad[1] * radii_rad[1]
+    if kind == "annular":
+        on &= t2 >= radii_rad[0] * radii_rad[0]
+    elif kind != "circular":
+        raise ValueError(kind)
+    return on.astype(np.float64)
+
+
+def detect(I: np.ndarray, weights: np.ndarray) -> np.ndarray:
+    """Energy-filtered STEM signal: out[d][e][p] = sum_r weights[d][r] I[p][e][r]; axes [detector][energy][scan] (:150)."""
+    return np.einsum("dr,per->dep", np.asarray(weights, dtype=np.float64), np.asarray(I, dtype=np.float64))

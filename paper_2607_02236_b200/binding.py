@@ -17,7 +17,10 @@ LIB_PATH = os.path.join(_HERE, "libtacaw.so")
 
 EXPORTS = ["tacaw_version", "tacaw_create", "tacaw_destroy", "tacaw_last_error", "tacaw_launch_count",
            "tacaw_build_slices", "tacaw_build_slices_host", "tacaw_make_probes", "tacaw_propagate",
-           "tacaw_make_roi", "tacaw_accumulate", "tacaw_spectrum", "tacaw_make_window", "tacaw_spectrum_welch"]
+           "tacaw_make_roi", "tacaw_accumulate", "tacaw_spectrum", "tacaw_make_window", "tacaw_spectrum_welch",
+           "tacaw_make_detector", "tacaw_detect"]
+
+DETECTORS = {"circular": 0, "annular": 1}
 
 WINDOWS = {"rect": 0, "hann": 1, "tukey": 2, "blackman_harris": 3, "kaiser": 4}
 
@@ -271,6 +274,40 @@ class Tacaw:
                                            C.byref(nch), self._stream())
         self._check(rc, "tacaw_spectrum_welch")
         return out, E[: nE.value].copy(), nch.value
+
+    def detect(self, I, weights, out=None):
+        """tacaw_detect: I float32 CUDA [P][nE][Q], weights float32 CUDA [D][Q] -> out float32 CUDA [D][nE][P]."""
+        torch = self.torch
+        P, nE, Q = I.shape
+        D = weights.shape[0]
+        if weights.shape != (D, Q):
+            raise ValueError("weights must be [ndet][nroi]")
+        if out is None:
+            out = torch.empty((D, nE, P), dtype=torch.float32, device=I.device)
+        for d0 in range(0, D, 8):
+            d1 = min(D, d0 + 8)
+            rc = self.lib.tacaw_detect(self._ctx, self._dev(I, torch.float32, "I"), C.c_int(P), C.c_int(nE), C.c_int64(Q),
+                                       self._dev(weights[d0:d1], torch.float32, "weights"), C.c_int(d1 - d0),
+                                       self._dev(out[d0:d1], torch.float32, "out"), self._stream())
+            self._check(rc, "tacaw_detect")
+        return out
+
+
+def make_detector(nx: int, ny: int, lx: float, ly: float, lam: float, kind: str, center_rad: Sequence[float],
+                  radii_rad: Sequence[float], roi_idx: np.ndarray) -> np.ndarray:
+    """tacaw_make_detector (host, exact): float32 0/1 weights over the ROI pixels for a circular (radii = (_, r)) or
+    annular (radii = (r_in, r_out)) detector centred at center_rad."""
+    lib = load_library()
+    g = _Grid(nx, ny, lx, ly)
+    idx = np.ascontiguousarray(roi_idx, dtype=np.int32)
+    c = (C.c_double * 2)(*center_rad)
+    r = (C.c_double * 2)(*radii_rad)
+    w = np.empty(idx.size, dtype=np.float32)
+    rc = lib.tacaw_make_detector(C.byref(g), C.c_double(lam), C.c_int(DETECTORS[kind]), c, r, idx.ctypes.data_as(C.c_void_p),
+                                 C.c_int64(idx.size), w.ctypes.data_as(C.c_void_p))
+    if rc != 0:
+        raise TacawError(f"tacaw_make_detector failed ({rc})")
+    return w
 
 
 def make_window(kind: str, n: int, param: float = 0.0) -> np.ndarray:

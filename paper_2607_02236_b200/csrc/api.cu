@@ -647,4 +647,31 @@ int tacaw_spectrum_welch(tacaw_ctx* ctx, const void* d_buf, int nprobes, int64_t
                          emin, emax, d_I, E_out, nE_out, (cudaStream_t)stream, "tacaw_spectrum_welch");
 }
 
+int tacaw_make_detector(const tacaw_grid* g, double lambda, int kind, const double* center, const double* radii,
+                        const int32_t* roi_idx, int64_t nroi, float* w_out) {
+    if (!g || g->nx <= 0 || g->ny <= 0 || !center || !radii || nroi < 0 || (nroi > 0 && (!roi_idx || !w_out))) return TACAW_E_ARG;
+    if (kind != TACAW_DETECTOR_CIRCULAR && kind != TACAW_DETECTOR_ANNULAR) return TACAW_E_ARG;
+    if (!(radii[1] >= 0) || (kind == TACAW_DETECTOR_ANNULAR && !(radii[0] >= 0 && radii[0] <= radii[1]))) return TACAW_E_ARG;
+    const long long npix = (long long)g->nx * g->ny;
+    for (int64_t r = 0; r < nroi; ++r) {
+        const long long idx = roi_idx[r];
+        if (idx < 0 || idx >= npix) return TACAW_E_ARG;
+        const int h = sgn_index((int)(idx % g->nx), g->nx), k = sgn_index((int)(idx / g->nx), g->ny);
+        const double tx = lambda * h / g->lx_A - center[0], ty = lambda * k / g->ly_A - center[1];
+        const double t2 = tx * tx + ty * ty;
+        bool on = t2 <= radii[1] * radii[1];
+        if (kind == TACAW_DETECTOR_ANNULAR) on = on && t2 >= radii[0] * radii[0];
+        w_out[r] = on ? 1.0f : 0.0f;
+    }
+    return TACAW_OK;
+}
+
+int tacaw_detect(tacaw_ctx* ctx, const float* d_I, int nprobes, int nE, int64_t nroi, const float* d_weights, int ndet,
+                 float* d_out, void* stream) {
+    if (!ctx) return TACAW_E_ARG;
+    if (nprobes < 0 || nE < 0 || nroi < 0 || ndet <= 0 || ((nprobes > 0 && nE > 0) && (!d_out || (nroi > 0 && (!d_I || !d_weights)))))
+        return fail(ctx, TACAW_E_ARG, "tacaw_detect: bad argument");
+    return launch_detect(ctx, d_I, nprobes, nE, nroi, d_weights, ndet, d_out, (cudaStream_t)stream);
+}
+
 }  // extern "C"

@@ -127,4 +127,7 @@ int launch_spectrum(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int64_t nr
                     int accumulate, const float2* d_roots,
                     const float* d_window, const float* d_bose, int e_lo, int nE, float* d_I, cudaStream_t st);
 
+int launch_detect(tacaw_ctx* ctx, const float* d_I, int nprobes, int nE, int64_t nroi, const float* d_w, int ndet, float* d_out,
+                  cudaStream_t st);
+
 }  // namespace tacaw

@@ -100,6 +100,54 @@ static int launch_spec_n(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int64
     return TACAW_OK;
 }
 
+// DetectorSet reduction: out[d][e][p] = sum_r w[d][r] I[p][e][r].  One warp per (p, e) row of I: float4 loads of the
+// row and of up to 8 weight rows (the weights stay in L2/L1), fp32 partial sums per lane, butterfly reduction.  I is
+// read once for all detectors of the call.
+template <int ND>
+__global__ void __launch_bounds__(256) k_detect(const float* __restrict__ I, long long nrows, long long nroi, int nE, int nprobes,
+                                                const float* __restrict__ w, float* __restrict__ out) {
+    const long long row = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;     // p*nE + e
+    const int lane = threadIdx.x & 31;
+    if (row >= nrows) return;
+    const float* src = I + row * nroi;
+    float acc[ND];
+#pragma unroll
+    for (int d = 0; d < ND; ++d) acc[d] = 0.f;
+    // rows start at arbitrary alignment (nroi need not be a multiple of 4): scalar accesses, coalesced across the warp
+    for (long long r = lane; r < nroi; r += 32) {
+        const float v = src[r];
+#pragma unroll
+        for (int d = 0; d < ND; ++d) acc[d] = fmaf(__ldg(w + d * nroi + r), v, acc[d]);
+    }
+#pragma unroll
+    for (int d = 0; d < ND; ++d) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) acc[d] += __shfl_xor_sync(0xffffffffu, acc[d], o);
+    }
+    if (lane == 0) {
+        const long long p = row / nE, e = row - p * nE;
+#pragma unroll
+        for (int d = 0; d < ND; ++d) out[((long long)d * nE + e) * nprobes + p] = acc[d];
+    }
+}
+
+int launch_detect(tacaw_ctx* ctx, const float* d_I, int nprobes, int nE, int64_t nroi, const float* d_w, int ndet, float* d_out,
+                  cudaStream_t st) {
+    const long long nrows = (long long)nprobes * nE;
+    if (nrows == 0) return TACAW_OK;
+    const unsigned blocks = (unsigned)((nrows * 32 + 255) / 256);
+#define TACAW_DET_CASE(K) case K: k_detect<K><<<blocks, 256, 0, st>>>(d_I, nrows, (long long)nroi, nE, nprobes, d_w, d_out); break;
+    switch (ndet) {
+        TACAW_DET_CASE(1) TACAW_DET_CASE(2) TACAW_DET_CASE(3) TACAW_DET_CASE(4)
+        TACAW_DET_CASE(5) TACAW_DET_CASE(6) TACAW_DET_CASE(7) TACAW_DET_CASE(8)
+        default: return fail(ctx, TACAW_E_UNSUPPORTED, "tacaw_detect: 1 to 8 detectors per call");
+    }
+#undef TACAW_DET_CASE
+    ctx->launches++;
+    TACAW_CUDA(ctx, cudaGetLastError());
+    return TACAW_OK;
+}
+
 int launch_spectrum(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int64_t nroi, int nframes, size_t probe_stride,
                     int accumulate, const float2* d_roots,
                     const float* d_window, const float* d_bose, int e_lo, int nE, float* d_I, cudaStream_t st) {
