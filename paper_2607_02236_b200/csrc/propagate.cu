@@ -15,6 +15,8 @@
 // by L1TEX (shared-memory wavefronts), so each 1D transform crosses shared memory once, wave rows and
 // columns go global <-> registers directly, and only what is reused (the t_n rows shared by the probes
 // of a frame, the Py table, the twiddles) is kept in shared memory.
+#include <cuda.h>
+
 #include <cstdlib>
 
 #include "ctx.h"
@@ -288,8 +290,8 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MINB) k_row(Row
 
 // Launch with programmatic dependent launch when asked: the kernel may start while its predecessor in the
 // stream drains; everything it does before pdl_wait() must not depend on that predecessor.
-template <class K, class A>
-static cudaError_t launch_pdl(K kern, unsigned grid, int threads, size_t smem, cudaStream_t st, bool pdl, const A& a) {
+template <class K, class... A>
+static cudaError_t launch_pdl(K kern, unsigned grid, int threads, size_t smem, cudaStream_t st, bool pdl, const A&... a) {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(grid);
     cfg.blockDim = dim3(threads);
@@ -304,7 +306,7 @@ static cudaError_t launch_pdl(K kern, unsigned grid, int threads, size_t smem, c
         return e ? atoi(e) != 0 : true;
     }();
     cfg.numAttrs = (pdl && pdl_on) ? 1 : 0;
-    return cudaLaunchKernelEx(&cfg, kern, a);
+    return cudaLaunchKernelEx(&cfg, kern, a...);
 }
 
 // grid that fills the machine exactly: occupancy x SM count CTAs
@@ -394,8 +396,10 @@ struct ColCfg {
     static constexpr int THREADS = T * WC;
     static constexpr int XE = exch2_elems(N, WC);
     static constexpr int MINB = (N <= 1024) ? 3 : 1;
-    // twiddles | Py | staging tile [N][WC] | exchange
-    static constexpr size_t smem() { return sizeof(float2) * ((size_t)P::TW_ELEMS + (PY_SMEM ? N : 0) + (size_t)N * WC + XE); }
+    // twiddles | Py | (pad to 128 B) staging tile [N][WC] (TMA destination) | exchange | mbarrier
+    static constexpr int OFF_S = ((P::TW_ELEMS + (PY_SMEM ? N : 0)) + 15) / 16 * 16;
+    static constexpr int RB = (N < 256) ? N : 256;            // rows per TMA box
+    static constexpr size_t smem() { return sizeof(float2) * ((size_t)OFF_S + (size_t)N * WC + XE + 2); }
 };
 
 // Work items of a column launch are (column group, wave) pairs, flattened as gi*nwaves + w over the
@@ -405,18 +409,23 @@ struct ColCfg {
 // BAND: every kmax[ix] <= N/3, so the chunks of k strictly between N/3 and N - N/3 are masked for
 // every column and are neither multiplied nor tested.
 template <int N, int MODE, bool BAND>
-__global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MINB) k_col(ColArgs a) {
+__global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MINB) k_col(ColArgs a, const __grid_constant__ CUtensorMap tm) {
     using C = ColCfg<N>;
     using P = Plan2<N>;
     constexpr int E = C::E, T = C::T, WC = C::WC;
-    extern __shared__ __align__(16) float2 smem[];
+    extern __shared__ __align__(128) float2 smem[];
     const int lt = threadIdx.x;
     const int c = lt % WC, tid = lt / WC;
     float2* tw = smem;
     float2* sPy = smem + P::TW_ELEMS;             // Py[ky]
-    float2* sS = sPy + (C::PY_SMEM ? N : 0);      // staging tile
+    float2* sS = smem + C::OFF_S;                 // staging tile
     float2* ex = sS + N * WC;
+    unsigned long long* bar = reinterpret_cast<unsigned long long*>(ex + C::XE);
     pdl_launch_dependents();
+    if (lt == 0) {
+        mbar_init(bar, 1);
+        mbar_init_fence();
+    }
     fft2_load_twiddles<N>(tw, a.roots, lt, C::THREADS);
     if constexpr (MODE != COL_INV && C::PY_SMEM) {
         for (int i = lt; i < N / 2; i += C::THREADS) cp_async16(sPy + 2 * i, a.py + 2 * i);
@@ -432,17 +441,17 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MINB) k_col(Col
     const long long i1 = min(i0 + (long long)a.ipc, a.nitems);
     const size_t npix = (size_t)N * a.nx;
     using B = Band<N, T, BAND>;
-    // tile of wave wv, column group grp -> staging: 16-byte chunks, E/2 per thread
+    // tile of wave wv, column group grp -> staging: one TMA box of [RB rows][WC columns] per RB rows, issued by one
+    // thread, completion counted in bytes on the mbarrier (every thread has passed a barrier after its last read of sS)
     auto issue_tile = [&](int wv, int grp) {
-        const float2* src = a.waves + (size_t)wv * npix + (size_t)grp * WC;
+        if (lt == 0) {
+            fence_proxy_async();
+            mbar_expect_tx(bar, (unsigned)(N * WC * sizeof(float2)));
 #pragma unroll
-        for (int j = 0; j < E / 2; ++j) {
-            const int id = lt + C::THREADS * j;
-            const int r = id / (WC / 2), part = id % (WC / 2);
-            cp_async16(sS + r * WC + 2 * part, src + (size_t)r * a.nx + 2 * part);
+            for (int b = 0; b < N / C::RB; ++b) tma_load_2d(sS + b * C::RB * WC, &tm, grp * WC, wv * N + b * C::RB, bar);
         }
-        cp_async_commit();
     };
+    unsigned parity = 0;
 
     auto body = [&](auto sync) {
         int gi = 0, w = 0;
@@ -478,6 +487,8 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MINB) k_col(Col
             }
             float2* wc = a.waves + (size_t)w * npix + coloff;
             const size_t rs = (size_t)T * a.nx;
+            mbar_wait(bar, parity);              // this item's tile has landed
+            parity ^= 1;
             float2 x[E];
 #pragma unroll
             for (int m = 0; m < E; ++m) {
@@ -503,27 +514,42 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MINB) k_col(Col
                     }
                 }
             }
-            if constexpr (MODE == COL_MID) {
-                // the barrier inside this exchange also publishes the prefetched tile
-                auto pre = [&]() { cp_async_wait_all(); };
-                NoHook post;
-                Hooks<decltype(pre), NoHook> hooks{pre, post};
-                fft2<N, WC, true, true>(x, twp, ex, tid, c, sync, hooks);
-            } else if constexpr (MODE == COL_INV) {
-                fft2<N, WC, true, false>(x, twp, ex, tid, c, sync);
-            }
+            if constexpr (MODE == COL_MID) fft2<N, WC, true, true>(x, twp, ex, tid, c, sync);
+            else if constexpr (MODE == COL_INV) fft2<N, WC, true, false>(x, twp, ex, tid, c, sync);
 #pragma unroll
             for (int m = 0; m < E; ++m) wc[m * rs] = x[m];
-            if constexpr (MODE != COL_MID) {
-                cp_async_wait_all();
-                sync();                          // prefetched tile visible
-            }
             w = wn;
             gi = gn;
         }
     };
     if constexpr (C::THREADS <= 32) body(SyncWarp{});
     else body(SyncBlock{});
+}
+
+// Tensor map of a stack of waves seen as a 2D array of 8-byte elements [rows][nx]; box = [box_rows][box_cols].
+static int make_tile_map(tacaw_ctx* ctx, CUtensorMap* tm, const void* base, int nx, long long rows, int box_cols, int box_rows) {
+    typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static encode_fn encode = [] {
+        void* f = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess) {
+            (void)cudaGetLastError();
+            f = nullptr;
+        }
+        return (encode_fn)f;
+    }();
+    if (!encode) return fail(ctx, TACAW_E_CUDA, "cuTensorMapEncodeTiled is not available");
+    const cuuint64_t dims[2] = {(cuuint64_t)nx, (cuuint64_t)rows};
+    const cuuint64_t strides[1] = {(cuuint64_t)nx * sizeof(float2)};
+    const cuuint32_t box[2] = {(cuuint32_t)box_cols, (cuuint32_t)box_rows};
+    const cuuint32_t estr[2] = {1, 1};
+    CUresult r = encode(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<void*>(base), dims, strides, box, estr,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(ctx, TACAW_E_CUDA, "cuTensorMapEncodeTiled failed (" + std::to_string((int)r) + ")");
+    return TACAW_OK;
 }
 
 // zero the out-of-band columns [c0, c1) of every row of every wave (exit wave Psi_S, O7)
@@ -558,7 +584,12 @@ static int launch_col_nb(tacaw_ctx* ctx, const ColArgs& a0, cudaStream_t st) {
     if (ctas > a.nitems) ctas = a.nitems;
     a.ipc = (int)((a.nitems + ctas - 1) / ctas);
     ctas = (a.nitems + a.ipc - 1) / a.ipc;
-    TACAW_CUDA(ctx, launch_pdl(kern, (unsigned)ctas, C::THREADS, smem, st, a.pdl != 0, a));
+    alignas(64) CUtensorMap tm;
+    {
+        int rc = make_tile_map(ctx, &tm, a.waves, a.nx, (long long)a.nwaves * N, C::WC, C::RB);
+        if (rc) return rc;
+    }
+    TACAW_CUDA(ctx, launch_pdl(kern, (unsigned)ctas, C::THREADS, smem, st, a.pdl != 0, a, tm));
     ctx->launches++;
     if (MODE == COL_LASTQ && !all) {
         const int c0 = nlo * C::WC, c1 = (NG - nhi) * C::WC;
