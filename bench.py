@@ -269,13 +269,16 @@ def main():
     e2e = None
     if not args.no_e2e:
         I_host = torch.empty(I.shape, dtype=I.dtype).pin_memory()
+        # the step's inputs live in pinned host memory (numpy views of pinned tensors)
+        pos_pin = [torch.from_numpy(p).pin_memory() for p in pos_h]
+        pos_hp = [t.numpy() for t in pos_pin]
         h2d = sum(p.nbytes for p in pos_h) + sum(s.nbytes for s in spec_h) * ((wl.nframes + r.fpb - 1) // r.fpb)
         d2h = I_host.numel() * 4
 
         def e2e_step():
             for f0 in range(0, wl.nframes, r.fpb):
                 nf = min(r.fpb, wl.nframes - f0)
-                r.build_block_host(pos_h, f0, nf)
+                r.build_block_host(pos_hp, f0, nf)
                 _, wp, wf = r.propagate_block(nf, 1)
                 r.gather_block(nf, f0, wp, wf)
             Ie, _ = r.spectrum()

@@ -143,18 +143,20 @@ __global__ void __launch_bounds__(POT_THREADS) k_potential(const uint32_t* __res
     if (h0 > hmax || kmax_pot[h0] < k0) return;        // tile entirely outside the mask
     const int lt = threadIdx.x;
     const int th = lt & 15, tk = lt >> 4;             // 16 x 8 threads, 2 (h) x 4 (k) points each
-    float4 acc[2][4], vs[2][4];
+    // per point two packed accumulators: P = (ac, ad) += a (c, d) and Q = (bc, bd) += b (c, d): two FFMA2 with a
+    // broadcast scalar operand instead of four FFMA (the kernel is bound by issue slots, not by the fp32 pipe)
+    float2 accP[2][4], accQ[2][4], vsP[2][4], vsQ[2][4];
 #pragma unroll
     for (int i = 0; i < 2; ++i)
 #pragma unroll
-        for (int j = 0; j < 4; ++j) vs[i][j] = make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int j = 0; j < 4; ++j) vsP[i][j] = vsQ[i][j] = make_float2(0.f, 0.f);
     for (int s = 0; s < nspecies; ++s) {
         const int a0 = offsets[n * nspecies + s], a1 = offsets[n * nspecies + s + 1];
         if (a0 == a1) continue;
 #pragma unroll
         for (int i = 0; i < 2; ++i)
 #pragma unroll
-            for (int j = 0; j < 4; ++j) acc[i][j] = make_float4(0.f, 0.f, 0.f, 0.f);
+            for (int j = 0; j < 4; ++j) accP[i][j] = accQ[i][j] = make_float2(0.f, 0.f);
         for (int base = a0; base < a1; base += POT_CHUNK) {
             const int cnt = min(POT_CHUNK, a1 - base);
             __syncthreads();
@@ -189,10 +191,8 @@ __global__ void __launch_bounds__(POT_THREADS) k_potential(const uint32_t* __res
                 for (int i = 0; i < 2; ++i)
 #pragma unroll
                     for (int j = 0; j < 4; ++j) {
-                        acc[i][j].x = fmaf(xh[i].x, yk[j].x, acc[i][j].x);
-                        acc[i][j].y = fmaf(xh[i].y, yk[j].y, acc[i][j].y);
-                        acc[i][j].z = fmaf(xh[i].x, yk[j].y, acc[i][j].z);
-                        acc[i][j].w = fmaf(xh[i].y, yk[j].x, acc[i][j].w);
+                        accP[i][j] = __ffma2_rn(yk[j], make_float2(xh[i].x, xh[i].x), accP[i][j]);
+                        accQ[i][j] = __ffma2_rn(yk[j], make_float2(xh[i].y, xh[i].y), accQ[i][j]);
                     }
             }
         }
@@ -205,10 +205,8 @@ __global__ void __launch_bounds__(POT_THREADS) k_potential(const uint32_t* __res
                 float f = 0.f;
 #pragma unroll
                 for (int g = 0; g < 4; ++g) f += ab.a[s][g] * expf(-ab.b[s][g] * q2);
-                vs[i][j].x = fmaf(f, acc[i][j].x, vs[i][j].x);
-                vs[i][j].y = fmaf(f, acc[i][j].y, vs[i][j].y);
-                vs[i][j].z = fmaf(f, acc[i][j].z, vs[i][j].z);
-                vs[i][j].w = fmaf(f, acc[i][j].w, vs[i][j].w);
+                vsP[i][j] = __ffma2_rn(accP[i][j], make_float2(f, f), vsP[i][j]);
+                vsQ[i][j] = __ffma2_rn(accQ[i][j], make_float2(f, f), vsQ[i][j]);
             }
     }
     float2* Vn = V + (size_t)n * nx * ny;
@@ -219,7 +217,7 @@ __global__ void __launch_bounds__(POT_THREADS) k_potential(const uint32_t* __res
             const int h = h0 + th + 16 * i, k = k0 + tk + 8 * j;
             if (h > hmax) continue;
             if (k > kmax_pot[h]) continue;
-            const float ac = vs[i][j].x, bd = vs[i][j].y, ad = vs[i][j].z, bc = vs[i][j].w;
+            const float ac = vsP[i][j].x, ad = vsP[i][j].y, bc = vsQ[i][j].x, bd = vsQ[i][j].y;
             const int ixm = (nx - h) % nx, iym = (ny - k) % ny;
             Vn[(size_t)k * nx + h] = make_float2(ac - bd, ad + bc);
             if (k > 0) Vn[(size_t)iym * nx + h] = make_float2(ac + bd, bc - ad);
