@@ -375,12 +375,16 @@ int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, const i
     // a slice step: all slices for group 0, then group 1, ...
     // a few groups are in flight at once (one per stream)
     size_t budget = ctx->l2_bytes ? ctx->l2_bytes / 4 : (size_t)32 << 20;
+    int gmin = 3;    // 2048^2: a launch over fewer waves is all fill and drain (measured: 1 wave 0.30, 3 waves 0.32 of the roofline)
     if (const char* e = getenv("TACAW_L2_GROUP_MB")) {
         double mb = atof(e);
-        if (mb > 0) budget = (size_t)(mb * 1048576.0);
+        if (mb > 0) {
+            budget = (size_t)(mb * 1048576.0);
+            gmin = 1;
+        }
     }
     int gmax = (int)(budget / (npix * sizeof(float2)));
-    if (gmax < 1) gmax = 1;
+    if (gmax < gmin) gmax = gmin;
     const int ngroups = (nwaves + gmax - 1) / gmax;
     static const int max_streams = [] {
         const char* e = getenv("TACAW_STREAMS");
