@@ -21,12 +21,23 @@ def _nvcc() -> str:
     raise RuntimeError("nvcc not found")
 
 
+def _source_hash() -> str:
+    """Hash of everything the library is built from (file names + contents + flags); mtimes do not survive a copy of the tree."""
+    import hashlib
+    h = hashlib.sha256(" ".join(NVCC_FLAGS).encode())
+    deps = sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC)) + [os.path.join(HERE, "..", "include", "tacaw.h")]
+    for d in deps:
+        h.update(os.path.basename(d).encode())
+        with open(d, "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()
+
+
 def _stale() -> bool:
-    if not os.path.exists(LIB):
+    if not os.path.exists(LIB) or not os.path.exists(LIB + ".hash"):
         return True
-    t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(HERE, "..", "include", "tacaw.h")]
-    return any(os.path.getmtime(d) > t for d in deps)
+    with open(LIB + ".hash") as fh:
+        return fh.read().strip() != _source_hash()
 
 
 def build_lib(force: bool = False, verbose: bool = False) -> str:
@@ -54,6 +65,8 @@ def build_lib(force: bool = False, verbose: bool = False) -> str:
     tmp = LIB + f".tmp{os.getpid()}"
     subprocess.check_call([nvcc, "-shared", "-cudart", "static", "-gencode", "arch=compute_100a,code=sm_100a", "-o", tmp, *objs])
     os.replace(tmp, LIB)
+    with open(LIB + ".hash", "w") as fh:
+        fh.write(_source_hash())
     return LIB
 
 
