@@ -44,8 +44,8 @@ struct tacaw_ctx {
     char* h_arena = nullptr;
     size_t arena_bytes = 0, arena_off = 0;
 
-    // second stream: tacaw_propagate runs alternate wave groups on it so one group's kernel tails
-    // overlap the other group's kernels (fork/join with events around the call)
+    // internal streams: tacaw_propagate runs wave groups round-robin on the caller's stream and these, so one group's
+    // kernel tails overlap the other groups' kernels (fork/join with events around the call; TACAW_STREAMS, default 3)
     static constexpr int MAX_AUX = 3;
     cudaStream_t aux[MAX_AUX] = {nullptr, nullptr, nullptr};
     cudaEvent_t ev_fork = nullptr, ev_join[MAX_AUX] = {nullptr, nullptr, nullptr};
