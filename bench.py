@@ -133,12 +133,28 @@ def oracle_sample(wl, nframes_sample: int):
     return steps / dt, dt, oracle.num_threads()
 
 
+def oracle_plan(args, wl):
+    """Bounded oracle sample: <= 4 probes and as many frames as give roughly 15 s of host work (--ref-frames overrides).
+    The estimate scales a measured 280 slice-steps/s (16 cores, 256^2) by the N^2 log N cost of a slice step."""
+    from paper_2607_02236_b200 import workloads as W
+    import math
+    npr = min(wl.nprobes, 4)
+    wls = wl if npr == wl.nprobes else W.make_workload(args.config, nframes=wl.nframes, nprobes=npr)
+    if args.ref_frames is not None:
+        nf = max(1, args.ref_frames)
+    else:
+        cores = max(1, min(16, len(os.sched_getaffinity(0))))
+        rate = 280.0 * (cores / 16.0) * (256.0 * 256.0 * 16.0) / (wl.nx * wl.ny * math.log2(wl.nx * wl.ny))
+        nf = int(max(1, min(wl.nframes, round(15.0 * rate / (npr * wl.nslices_total)))))
+    return wls, nf
+
+
 def run_reference(args, wl):
     """--impl reference: the fp64 oracle on host cores, bounded sample per step."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    nf = max(1, args.ref_frames)
+    wl, nf = oracle_plan(args, wl)
     for _ in range(args.warmup):
         oracle_sample(wl, 1)
     vals, times = [], []
@@ -165,7 +181,7 @@ def main():
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number 1..5 (default 2 = configs[1])")
     ap.add_argument("--frames", type=int, default=None, help="truncate the workload to its first FRAMES frames")
     ap.add_argument("--probes", type=int, default=None, help="truncate the workload to its first PROBES probes")
-    ap.add_argument("--ref-frames", type=int, default=2, help="frames per step of the oracle sample")
+    ap.add_argument("--ref-frames", type=int, default=None, help="frames per step of the oracle sample (default: ~15 s of host work)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -316,9 +332,10 @@ def main():
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        v, dt, cores = oracle_sample(wl, max(1, args.ref_frames))
+        wls, nfs = oracle_plan(args, wl)
+        v, dt, cores = oracle_sample(wls, nfs)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": f"{max(1, args.ref_frames)} frame(s) x {wl.nprobes} probes x {wl.nslices_total} slices of {wl.name} "
+               "sample": f"{nfs} frame(s) x {wls.nprobes} probes x {wl.nslices_total} slices of {wl.name} "
                          f"(build + propagate), {dt:.1f} s"}
 
     if rank == 0:
