@@ -205,6 +205,8 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
     shard_workload(wl, rank)          # every rank = its own scan batch of the same size
 
+    from paper_2607_02236_b200 import build as _build
+    _build.build_lib()                # no-op when libtacaw.so matches the sources; never a fallback: it raises if nvcc fails
     from paper_2607_02236_b200.pipeline import Runner
     r = Runner(wl, device=local_rank)
     r.alloc_buffer()

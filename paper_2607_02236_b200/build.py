@@ -43,6 +43,16 @@ def _stale() -> bool:
 def build_lib(force: bool = False, verbose: bool = False) -> str:
     if not force and not _stale():
         return LIB
+    # one builder at a time (ranks of a torchrun job start together); the others find a fresh library afterwards
+    import fcntl
+    with open(os.path.join(HERE, ".build.lock"), "w") as lock:
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        if not force and not _stale():
+            return LIB
+        return _build_locked(verbose)
+
+
+def _build_locked(verbose: bool) -> str:
     nvcc = _nvcc()
     os.makedirs(os.path.join(HERE, "build"), exist_ok=True)
     objs = [os.path.join(HERE, "build", s.replace(".cu", ".o")) for s in SOURCES]
