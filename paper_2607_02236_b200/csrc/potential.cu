@@ -166,6 +166,7 @@ __global__ void __launch_bounds__(POT_THREADS) k_potential(const uint32_t* __res
                     const int axis = e / 12, j = e % 12;
                     const uint32_t u = axis ? sy[base + at] : sx[base + at];
                     if (j < 4) coarse[axis][j][at] = phase_fixed(u, (axis ? k0 : h0) + 8 * j);
+                    else if (j == 4) fine[axis][0][at] = make_float2(1.f, 0.f);        // exp(0)
                     else fine[axis][j - 4][at] = phase_fixed(u, j - 4);
                 }
             }
@@ -175,7 +176,9 @@ __global__ void __launch_bounds__(POT_THREADS) k_potential(const uint32_t* __res
                 if (at < cnt) {
                     const int axis = rr / POT_T, r = rr % POT_T;
                     const float2 cph = coarse[axis][r >> 3][at], fph = fine[axis][r & 7][at];
-                    const float2 ph = make_float2(cph.x * fph.x - cph.y * fph.y, cph.x * fph.y + cph.y * fph.x);
+                    // packed complex product (FMUL2 + FFMA2)
+                    const float2 ph = __ffma2_rn(make_float2(-cph.y, cph.x), make_float2(fph.y, fph.y),
+                                                 __fmul2_rn(cph, make_float2(fph.x, fph.x)));
                     if (axis) ey[r][at] = ph; else ex[r][at] = ph;
                 }
             }
