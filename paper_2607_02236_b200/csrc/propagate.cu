@@ -387,11 +387,14 @@ int launch_row(tacaw_ctx* ctx, int mode, const RowArgs& a, cudaStream_t st) {
 }
 
 // ------------------------------------------------------------------------------------------
-template <int N>
+template <int N, int MODE = COL_MID>
 struct ColCfg {
     using P = Plan2<N>;
     static constexpr int E = P::E, T = P::T;
-    static constexpr int WC = (N >= 1024) ? 4 : 8;          // adjacent columns transformed together
+    // adjacent columns transformed together.  The slice step reads its tiles from L2, where 64-byte row segments are
+    // full speed; the potential pass (COL_INV at 256^2 and below) streams from HBM, where they cost a 2x over-fetch
+    // (ncu: 7.4 GB read for 3.7 GB of tiles), so it takes full 128-byte lines
+    static constexpr int WC = (N >= 1024) ? 4 : ((MODE == COL_INV && N <= 256) ? 16 : 8);
     static constexpr bool PY_SMEM = (N <= 512);              // Py table in shared memory (else read through L1)
     static constexpr int THREADS = T * WC;
     static constexpr int XE = exch2_elems(N, WC);
@@ -409,8 +412,8 @@ struct ColCfg {
 // BAND: every kmax[ix] <= N/3, so the chunks of k strictly between N/3 and N - N/3 are masked for
 // every column and are neither multiplied nor tested.
 template <int N, int MODE, bool BAND>
-__global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MINB) k_col(ColArgs a, const __grid_constant__ CUtensorMap tm) {
-    using C = ColCfg<N>;
+__global__ void __launch_bounds__(ColCfg<N, MODE>::THREADS, ColCfg<N, MODE>::MINB) k_col(ColArgs a, const __grid_constant__ CUtensorMap tm) {
+    using C = ColCfg<N, MODE>;
     using P = Plan2<N>;
     constexpr int E = C::E, T = C::T, WC = C::WC;
     extern __shared__ __align__(128) float2 smem[];
@@ -565,7 +568,7 @@ __global__ void k_zero_cols(float2* __restrict__ waves, long long nrows, int nx,
 
 template <int N, int MODE, bool BAND>
 static int launch_col_nb(tacaw_ctx* ctx, const ColArgs& a0, cudaStream_t st) {
-    using C = ColCfg<N>;
+    using C = ColCfg<N, MODE>;
     ColArgs a = a0;
     const int NG = a.nx / C::WC;
     const int nlo = a.hmax / C::WC + 1, nhi = (a.hmax + C::WC - 1) / C::WC;
