@@ -189,6 +189,31 @@ int tacaw_make_detector(const tacaw_grid *grid, double lambda_A, int kind, const
 int tacaw_detect(tacaw_ctx *ctx, const float *d_I, int nprobes, int nE, int64_t nroi, const float *d_weights, int ndet,
                  float *d_out, void *stream);
 
+/* Scan grids ("four different scanning modes: 'unitcell', 'box', 'box_relative', and 'parallelogram'
+ * ... over a two dimensional grid with grid shape defined by the user explicitly ... the end point is by design
+ * not included -- 5 scan points on [0.0, 1.0) give {0.0, 0.2, 0.4, 0.6, 0.8}"; Listing 1 :416-428; SURVEY.md 8(f)
+ * item 4; reading G23 of DESIGN.md).  HOST, fp64.  Point (i, j), i < shape[0], j < shape[1], is row
+ * p = i*shape[1] + j of xy_out, ready for tacaw_make_probes:
+ *   BOX           r = origin + (i/n0 (a_x - o_x), j/n1 (a_y - o_y)),  a = far corner of the box [A]; b, cell unused
+ *   BOX_RELATIVE  the same with origin and a as fractions of the simulation cell, cell = {lx_A, ly_A}; b unused
+ *   UNITCELL      r = origin + (i/n0 a_x, j/n1 a_y),  a = edge lengths of one unit cell [A]; b, cell unused
+ *   PARALLELOGRAM r = origin + (i/n0) a + (j/n1) b,   a, b = edge vectors [A]; cell unused
+ * xy_out HOST double [shape[0]*shape[1]][2].  Returns TACAW_E_ARG on a bad mode, a non-positive shape or a missing
+ * array. */
+#define TACAW_SCAN_BOX 0
+#define TACAW_SCAN_BOX_RELATIVE 1
+#define TACAW_SCAN_UNITCELL 2
+#define TACAW_SCAN_PARALLELOGRAM 3
+int tacaw_make_scan(int mode, const int32_t *shape, const double *origin, const double *a, const double *b,
+                    const double *cell, double *xy_out);
+
+/* Scan sub-batches ("scan sub-batch", Listing 1 :428 scanning_batch_shape): the scan grid is cut into tiles
+ * of batch_shape[0] x batch_shape[1] points (ragged at the far edges), numbered row-major over the tile grid; tile
+ * `batch` lists its scan rows p = i*shape[1] + j in ascending (i, j).  HOST.  idx_out NULL: count only.
+ * nbatches (may be NULL) receives the number of tiles.  batch outside [0, nbatches) is TACAW_E_ARG. */
+int tacaw_scan_batch(const int32_t *shape, const int32_t *batch_shape, int batch, int32_t *idx_out, int32_t *count,
+                     int32_t *nbatches);
+
 /* Convenience for host-resident data (bench.py's end-to-end leg): same as the calls above but the
  * named buffers are HOST memory; the library stages them through its own device scratch with
  * cudaMemcpyAsync on `stream` and synchronises before returning. */

@@ -309,3 +309,53 @@ def detector_weights(nx: int, ny: int, lx: float, ly: float, lam: float, kind: s
 def detect(I: np.ndarray, weights: np.ndarray) -> np.ndarray:
     """Energy-filtered STEM signal: out[d][e][p] = sum_r weights[d][r] I[p][e][r]; axes [detector][energy][scan] (:150)."""
     return np.einsum("dr,per->dep", np.asarray(weights, dtype=np.float64), np.asarray(I, dtype=np.float64))
+
+
+# SURVEY.md 8(f) item 4 (workload variants): scan grids (PAPER.md:378-380, Listing 1 :416-428).
+
+def scan_positions(mode: str, shape: Sequence[int], origin: Sequence[float], a: Sequence[float],
+                   b: Optional[Sequence[float]] = None, cell: Optional[Sequence[float]] = None) -> np.ndarray:
+    """The four scanning modes (:378).  'the scanning is performed over a two dimensional grid with grid shape ...
+    defined by the user explicitly.  Note that the end point is by design "not included" -- for example, 5 scan
+    points on interval [0.0, 1.0) would result in points {0.0, 0.2, 0.4, 0.6, 0.8}' (:378-380).
+    Point (i, j), i < shape[0], j < shape[1], row p = i*shape[1] + j (reading G23):
+      'box'           r = origin + (i/n0 (a_x - o_x), j/n1 (a_y - o_y));   a = scanning_box_end [A]  (:419-424)
+      'box_relative'  the same with origin and a given as fractions of the simulation cell (cell = lx, ly [A])
+      'unitcell'      box from origin over one unit cell with edges a = (a_uc, b_uc) [A]
+      'parallelogram' r = origin + (i/n0) a + (j/n1) b;   a, b edge vectors [A]
+    Plain loops, no vectorisation."""
+    n0, n1 = int(shape[0]), int(shape[1])
+    out = np.zeros((n0 * n1, 2), dtype=np.float64)
+    for i in range(n0):
+        for j in range(n1):
+            fi, fj = i / n0, j / n1
+            if mode == "box":
+                x = origin[0] + fi * (a[0] - origin[0])
+                y = origin[1] + fj * (a[1] - origin[1])
+            elif mode == "box_relative":
+                x = (origin[0] + fi * (a[0] - origin[0])) * cell[0]
+                y = (origin[1] + fj * (a[1] - origin[1])) * cell[1]
+            elif mode == "unitcell":
+                x = origin[0] + fi * a[0]
+                y = origin[1] + fj * a[1]
+            elif mode == "parallelogram":
+                x = origin[0] + fi * a[0] + fj * b[0]
+                y = origin[1] + fi * a[1] + fj * b[1]
+            else:
+                raise ValueError(mode)
+            out[i * n1 + j] = (x, y)
+    return out
+
+
+def scan_batches(shape: Sequence[int], batch_shape: Sequence[int]) -> List[np.ndarray]:
+    """Scan sub-batches (:131 'scan sub-batch', Listing 1 :428 scanning_batch_shape = [4, 8] for a 16 x 16 scan): the
+    scan grid is cut into tiles of batch_shape[0] x batch_shape[1] points (ragged at the far edges); tiles are numbered
+    row-major over the tile grid and each lists its scan rows p = i*shape[1] + j in ascending (i, j)."""
+    n0, n1 = int(shape[0]), int(shape[1])
+    b0, b1 = int(batch_shape[0]), int(batch_shape[1])
+    tiles = []
+    for ti in range(0, n0, b0):
+        for tj in range(0, n1, b1):
+            tiles.append(np.array([i * n1 + j for i in range(ti, min(ti + b0, n0)) for j in range(tj, min(tj + b1, n1))],
+                                  dtype=np.int32))
+    return tiles

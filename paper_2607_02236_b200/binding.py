@@ -18,9 +18,11 @@ LIB_PATH = os.path.join(_HERE, "libtacaw.so")
 EXPORTS = ["tacaw_version", "tacaw_create", "tacaw_destroy", "tacaw_last_error", "tacaw_launch_count",
            "tacaw_build_slices", "tacaw_build_slices_host", "tacaw_make_probes", "tacaw_propagate",
            "tacaw_make_roi", "tacaw_accumulate", "tacaw_spectrum", "tacaw_make_window", "tacaw_spectrum_welch",
-           "tacaw_make_detector", "tacaw_detect"]
+           "tacaw_make_detector", "tacaw_detect", "tacaw_make_scan", "tacaw_scan_batch"]
 
 DETECTORS = {"circular": 0, "annular": 1}
+
+SCAN_MODES = {"box": 0, "box_relative": 1, "unitcell": 2, "parallelogram": 3}
 
 WINDOWS = {"rect": 0, "hann": 1, "tukey": 2, "blackman_harris": 3, "kaiser": 4}
 
@@ -318,3 +320,33 @@ def make_window(kind: str, n: int, param: float = 0.0) -> np.ndarray:
     if rc != 0:
         raise TacawError(f"tacaw_make_window failed ({rc})")
     return w
+
+
+def make_scan(mode: str, shape: Sequence[int], origin: Sequence[float], a: Sequence[float],
+              b: Optional[Sequence[float]] = None, cell: Optional[Sequence[float]] = None) -> np.ndarray:
+    """tacaw_make_scan (host): scan positions [shape[0]*shape[1]][2] in Angstrom, end point excluded."""
+    lib = load_library()
+    sh = (C.c_int32 * 2)(*[int(v) for v in shape])
+    d2 = lambda v: None if v is None else (C.c_double * 2)(*[float(x) for x in v])
+    n = max(int(shape[0]), 0) * max(int(shape[1]), 0)
+    xy = np.empty((n, 2), dtype=np.float64)
+    rc = lib.tacaw_make_scan(C.c_int(SCAN_MODES[mode]), sh, d2(origin), d2(a), d2(b), d2(cell), xy.ctypes.data_as(C.c_void_p))
+    if rc != 0:
+        raise TacawError(f"tacaw_make_scan failed ({rc})")
+    return xy
+
+
+def scan_batch(shape: Sequence[int], batch_shape: Sequence[int], batch: int) -> Tuple[np.ndarray, int]:
+    """tacaw_scan_batch (host): scan rows of sub-batch `batch` and the number of sub-batches."""
+    lib = load_library()
+    sh = (C.c_int32 * 2)(*[int(v) for v in shape])
+    bs = (C.c_int32 * 2)(*[int(v) for v in batch_shape])
+    cnt, nb = C.c_int32(0), C.c_int32(0)
+    rc = lib.tacaw_scan_batch(sh, bs, C.c_int(batch), None, C.byref(cnt), C.byref(nb))
+    if rc != 0:
+        raise TacawError(f"tacaw_scan_batch failed ({rc})")
+    idx = np.empty(cnt.value, dtype=np.int32)
+    rc = lib.tacaw_scan_batch(sh, bs, C.c_int(batch), idx.ctypes.data_as(C.c_void_p), C.byref(cnt), C.byref(nb))
+    if rc != 0:
+        raise TacawError(f"tacaw_scan_batch failed ({rc})")
+    return idx, nb.value

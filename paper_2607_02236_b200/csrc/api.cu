@@ -651,6 +651,50 @@ int tacaw_spectrum_welch(tacaw_ctx* ctx, const void* d_buf, int nprobes, int64_t
                          emin, emax, d_I, E_out, nE_out, (cudaStream_t)stream, "tacaw_spectrum_welch");
 }
 
+int tacaw_make_scan(int mode, const int32_t* shape, const double* origin, const double* a, const double* b, const double* cell,
+                    double* xy_out) {
+    if (!shape || !origin || !a || !xy_out || shape[0] <= 0 || shape[1] <= 0) return TACAW_E_ARG;
+    if (mode < TACAW_SCAN_BOX || mode > TACAW_SCAN_PARALLELOGRAM) return TACAW_E_ARG;
+    if ((mode == TACAW_SCAN_PARALLELOGRAM && !b) || (mode == TACAW_SCAN_BOX_RELATIVE && !cell)) return TACAW_E_ARG;
+    const int n0 = shape[0], n1 = shape[1];
+    // edge vectors e0 (along i) and e1 (along j) and the start corner, in Angstrom; end point excluded (:380)
+    double o[2] = {origin[0], origin[1]}, e0[2] = {0.0, 0.0}, e1[2] = {0.0, 0.0};
+    switch (mode) {
+        case TACAW_SCAN_BOX: e0[0] = a[0] - origin[0]; e1[1] = a[1] - origin[1]; break;
+        case TACAW_SCAN_UNITCELL: e0[0] = a[0]; e1[1] = a[1]; break;
+        case TACAW_SCAN_PARALLELOGRAM: e0[0] = a[0]; e0[1] = a[1]; e1[0] = b[0]; e1[1] = b[1]; break;
+        default: break;
+    }
+    for (int i = 0; i < n0; ++i)
+        for (int j = 0; j < n1; ++j) {
+            const double fi = (double)i / (double)n0, fj = (double)j / (double)n1;
+            double* r = xy_out + 2 * ((size_t)i * n1 + j);
+            if (mode == TACAW_SCAN_BOX_RELATIVE) {
+                r[0] = (origin[0] + fi * (a[0] - origin[0])) * cell[0];
+                r[1] = (origin[1] + fj * (a[1] - origin[1])) * cell[1];
+            } else {
+                r[0] = o[0] + fi * e0[0] + fj * e1[0];
+                r[1] = o[1] + fi * e0[1] + fj * e1[1];
+            }
+        }
+    return TACAW_OK;
+}
+
+int tacaw_scan_batch(const int32_t* shape, const int32_t* bs, int batch, int32_t* idx_out, int32_t* count, int32_t* nbatches) {
+    if (!shape || !bs || !count || shape[0] <= 0 || shape[1] <= 0 || bs[0] <= 0 || bs[1] <= 0) return TACAW_E_ARG;
+    const int t0 = (shape[0] + bs[0] - 1) / bs[0], t1 = (shape[1] + bs[1] - 1) / bs[1];
+    if (nbatches) *nbatches = t0 * t1;
+    if (batch < 0 || batch >= t0 * t1) return TACAW_E_ARG;
+    const int i0 = (batch / t1) * bs[0], j0 = (batch % t1) * bs[1];
+    const int i1 = i0 + bs[0] < shape[0] ? i0 + bs[0] : shape[0], j1 = j0 + bs[1] < shape[1] ? j0 + bs[1] : shape[1];
+    int32_t c = 0;
+    for (int i = i0; i < i1; ++i)
+        for (int j = j0; j < j1; ++j, ++c)
+            if (idx_out) idx_out[c] = i * shape[1] + j;
+    *count = c;
+    return TACAW_OK;
+}
+
 int tacaw_make_detector(const tacaw_grid* g, double lambda, int kind, const double* center, const double* radii,
                         const int32_t* roi_idx, int64_t nroi, float* w_out) {
     if (!g || g->nx <= 0 || g->ny <= 0 || !center || !radii || nroi < 0 || (nroi > 0 && (!roi_idx || !w_out))) return TACAW_E_ARG;

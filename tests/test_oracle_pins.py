@@ -18,7 +18,8 @@ def golden():
         if line.startswith("#") or not line.strip():
             continue
         k, v, _cite = [s.strip() for s in line.split("|", 2)]
-        out[k] = float(v)
+        vals = [float(x) for x in v.split()]
+        out[k] = vals[0] if len(vals) == 1 else vals
     return out
 
 
