@@ -320,7 +320,15 @@ static int machine_ctas(const tacaw_ctx* ctx, K kern, int threads, size_t smem, 
         }
         *cache = per_sm;
     }
-    return ctx->num_sms * (*cache);
+    // TACAW_GRID_FRAC (tuning knob, default 1): launch only this fraction of the machine-filling grid, so that kernels of
+    // different streams share the machine side by side instead of one after the other
+    static const double frac = [] {
+        const char* e = getenv("TACAW_GRID_FRAC");
+        const double v = e ? atof(e) : 1.0;
+        return (v > 0.0 && v <= 1.0) ? v : 1.0;
+    }();
+    const int n = (int)(ctx->num_sms * (*cache) * frac);
+    return n < 1 ? 1 : n;
 }
 
 template <int N, int MODE, bool BAND>
