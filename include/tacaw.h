@@ -117,7 +117,8 @@ int tacaw_make_probes(tacaw_ctx *ctx, const double *probe_xy_A, int nprobes, dou
  * output_space 0: r-space psi_S;  1: q-space Psi_S = FFT2(psi_S), unnormalised, native FFT order. */
 /* Tuning knobs of tacaw_propagate, read from the environment (defaults swept on B200):
  *   TACAW_STREAMS=n        wave groups in flight, caller's stream + n-1 internal ones (default 3, max 4; read once)
- *   TACAW_L2_GROUP_MB=x    bytes of full waves per group (default L2/4, at least 3 waves)
+ *   TACAW_L2_GROUP_MB=x    bytes of full waves per group (default L2/5, whole row tuples, at least 3 waves)
+ *   TACAW_GRID_FRAC=f      fraction of the machine-filling grid a slice-step launch uses (default 1; 0.5-1 measured equal)
  *   TACAW_PDL=0            launch the slice-step kernels without programmatic dependent launch
  * They change scheduling only, never results (tests/test_gpu_parity.py::test_propagate_l2_grouping_is_transparent). */
 int tacaw_propagate(tacaw_ctx *ctx, void *d_waves, const void *d_probes, const int32_t *wave_probe,

@@ -374,7 +374,9 @@ int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, const i
     // depth-first over groups of waves small enough to stay L2-resident between the two kernels of
     // a slice step: all slices for group 0, then group 1, ...
     // a few groups are in flight at once (one per stream)
-    size_t budget = ctx->l2_bytes ? ctx->l2_bytes / 4 : (size_t)32 << 20;
+    // L2/5 (25 MB: 48 waves at 256^2, 12 at 512^2, 3 at 1024^2), swept on B200: 512^2 reaches 0.556 of the roofline with
+    // 12 waves per group, 0.54 with 15 (L2/4), 0.53 with 11
+    size_t budget = ctx->l2_bytes ? ctx->l2_bytes / 5 : (size_t)25 << 20;
     int gmin = 3;    // 2048^2: a launch over fewer waves is all fill and drain (measured: 1 wave 0.30, 3 waves 0.32 of the roofline)
     if (const char* e = getenv("TACAW_L2_GROUP_MB")) {
         double mb = atof(e);
@@ -384,6 +386,7 @@ int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, const i
         }
     }
     int gmax = (int)(budget / (npix * sizeof(float2)));
+    if (gmax >= 2 * rpt) gmax -= gmax % rpt;      // whole row tuples: a short tuple repeats its last wave (wasted work)
     if (gmax < gmin) gmax = gmin;
     const int ngroups = (nwaves + gmax - 1) / gmax;
     static const int max_streams = [] {
