@@ -394,3 +394,85 @@ def test_config5_thin_sampled(torch, B, oracle):
     """configs[4] shape (2048^2, planar fault, annular ROI), 2 cells thick."""
     wl = W.make_workload(5, ncz=2)
     assert _exit_wave_parity(torch, oracle, wl, [1500], probes=[5]) <= TOL_WAVE
+
+
+# ------------------------------------------------------------------- degenerate and empty inputs
+def test_free_space_is_analytic_fresnel_on_the_gpu(torch, B, oracle):
+    """No atoms: t = 1 and S slice steps must give FFT2(psi_S) = Psi_0 exp(-i pi lambda S dz q^2) inside the mask, 0 outside
+    (DESIGN.md pin P1a, here for the CUDA path itself and against the oracle)."""
+    n, L, lam, dz, S = 128, 18.376, 0.0370144, 1.4795, 7
+    tc = B.Tacaw(n, n, L, L, lam, 9.2e-4, 1)
+    a = np.array([[100.0, 50.0, 20.0, 5.0]])
+    b = np.array([[0.3, 1.0, 3.0, 8.0]])
+    pos = torch.zeros((0, 3), dtype=torch.float64, device="cuda")
+    sp = torch.zeros((0,), dtype=torch.int32, device="cuda")
+    t, ncl = tc.build_slices(pos, sp, a, b, dz, S, 0.0, want_clamped=True)
+    assert ncl == 0 and torch.all(t == 1)
+    xy = np.array([[3.1, 7.7], [0.0, 0.0]])
+    psi0 = tc.make_probes(xy, 30e-3)
+    q0 = torch.fft.fft2(psi0).cpu().numpy().astype(np.complex128)          # library FFT: test-side check only
+    waves = psi0.clone()
+    tc.propagate(waves, [0, 0], [[t]], dz, 1)
+    got = waves.cpu().numpy().astype(np.complex128)
+    h = np.fft.fftfreq(n, 1.0 / n)
+    hh, kk = np.meshgrid(h, h, indexing="xy")
+    q2 = (hh ** 2 + kk ** 2) / L ** 2
+    mask = 9 * (hh ** 2 + kk ** 2) <= n * n
+    expect = q0 * np.exp(-1j * np.pi * lam * S * dz * q2) * mask
+    ref = oracle.propagate(L, L, lam, 1, psi0.cpu().numpy().astype(np.complex128), np.array([0, 0], np.int32),
+                           [[np.ones((S, n, n), complex)]], dz, 1)
+    for p in range(2):
+        assert rel_l2(got[p], expect[p]) <= 2e-5
+        assert rel_l2(got[p], ref[p]) <= 2e-5
+        assert np.all(got[p][~mask] == 0)
+    tc.close()
+
+
+def test_empty_slice_between_occupied_ones(torch, B, oracle):
+    """A slice that holds no atom has t_n = 1 exactly; its neighbours are unaffected."""
+    wl = W.tiny_workload(n=32, ncell=(1, 1, 2))
+    seg = wl.segments[0]
+    pos = seg.pos0.copy()
+    pos[:, 2] = np.where(pos[:, 2] < 2.0 * wl.dz, 0.5 * wl.dz, 2.5 * wl.dz)     # slices 0 and 2 occupied, 1 and 3 empty
+    ref = oracle.build_slices(wl.nx, wl.ny, wl.lx, wl.ly, pos, seg.species, wl.a, wl.b, wl.dz, 4, 0.0, wl.sigma, 1, 1)
+    tc = B.Tacaw(wl.nx, wl.ny, wl.lx, wl.ly, wl.lam, wl.sigma, 1)
+    t, ncl = tc.build_slices(dev(torch, pos), dev(torch, seg.species), wl.a, wl.b, wl.dz, 4, 0.0, want_clamped=True)
+    assert ncl == 0
+    assert torch.all(t[1] == 1) and torch.all(t[3] == 1)
+    assert rel_l2(t.cpu().numpy(), ref["trans"]) <= 1e-5
+    tc.close()
+
+
+def test_empty_batches_are_no_ops(torch, B):
+    n = 32
+    tc = B.Tacaw(n, n, 5.0, 5.0, 0.037, 9e-4, 1)
+    roi = B.make_roi(n, n, 5.0, 5.0, 0.037, "disc", [0.05])
+    q = torch.randn((2, n, n), dtype=torch.complex64, device="cuda")
+    buf = torch.full((1, 2, roi.size), 7.0, dtype=torch.complex64, device="cuda")
+    tc.accumulate(q[:0], [], [], dev(torch, roi), buf)                           # no waves
+    assert torch.all(buf == 7.0)
+    empty_roi = torch.zeros((0,), dtype=torch.int32, device="cuda")
+    buf0 = torch.zeros((1, 2, 0), dtype=torch.complex64, device="cuda")
+    tc.accumulate(q, [0, 0], [0, 1], empty_roi, buf0)                            # empty ROI
+    I, E = tc.spectrum(torch.zeros((0, 16, 5), dtype=torch.complex64, device="cuda"), 5.0, 1, 300.0)   # no probes
+    assert I.shape == (0, 16, 5) and E.size == 16
+    I, E = tc.spectrum(torch.zeros((2, 16, 0), dtype=torch.complex64, device="cuda"), 5.0, 1, 300.0)   # no pixels
+    assert I.shape == (2, 16, 0)
+    assert tc.make_probes(np.zeros((0, 2)), 30e-3).shape == (0, n, n)
+    torch.cuda.synchronize()
+    tc.close()
+
+
+def test_single_series_single_pixel_spectrum(torch, B, oracle):
+    """P = Q = 1: one series alone in its tile; a pure tone on a bin gives one line scaled by the Bose factor."""
+    T, dt = 64, 5.0
+    f = np.arange(T)
+    buf = (np.exp(2j * np.pi * 5 * f / T) + 0.25 * np.exp(-2j * np.pi * 9 * f / T)).reshape(1, T, 1)
+    tc = B.Tacaw(16, 16, 5.0, 5.0, 0.037, 9e-4, 1)
+    I, E = tc.spectrum(dev(torch, buf, torch.complex64), dt, 0, 300.0)
+    Iref, Eref = oracle.spectrum(buf, dt, 0, 300.0)
+    got = I.cpu().numpy()
+    assert np.array_equal(E, Eref) and rel_l2(got, Iref) <= 5e-6
+    top = np.argsort(got[0, :, 0])[-2:]
+    assert sorted(top.tolist()) == sorted([T // 2 + 5, T // 2 - 9])
+    tc.close()
