@@ -553,20 +553,28 @@ static int spectrum_core(tacaw_ctx* ctx, const void* d_buf, int nprobes, int64_t
     if (E_out) for (int i = 0; i < nE; ++i) E_out[i] = E[i];
     if (!d_I || nE == 0 || nprobes == 0 || nroi == 0 || nchunks == 0) return TACAW_OK;
     if (!d_buf) return fail(ctx, TACAW_E_ARG, std::string(who) + ": null buffer");
-    std::vector<float> tab(2 * (size_t)L + (size_t)L + (size_t)nE);   // roots (float2 x L), window, bose
+    // table region: roots exp(-2 pi i j/L) (L < 512) or the single-exchange twiddle table of fft2.cuh (L >= 512); window; bose
+    static const bool two_exchange = [] { const char* e = getenv("TACAW_SPEC_TWO_EXCHANGE"); return e && atoi(e) != 0; }();
+    const bool plan2 = L >= 512 && !two_exchange;
+    const size_t ntw = plan2 ? (size_t)fft2_table_elems(L) : (size_t)L;
+    const size_t NR = ntw > (size_t)L ? ntw : (size_t)L;               // float2 entries reserved for the table
+    std::vector<float> tab(2 * NR + (size_t)L + (size_t)nE);
     double sw2 = 0.0;
     for (int f = 0; f < L; ++f) sw2 += w[f] * w[f];
     if (!(sw2 > 0)) return fail(ctx, TACAW_E_ARG, std::string(who) + ": window is identically zero");
+    if (plan2) fft2_host_table(L, reinterpret_cast<float2*>(tab.data()));
     for (int j = 0; j < L; ++j) {
-        double ang = -2.0 * M_PI * (double)j / (double)L;
-        tab[2 * j] = (float)std::cos(ang);
-        tab[2 * j + 1] = (float)std::sin(ang);
-        tab[2 * (size_t)L + j] = (float)w[j];
+        if (!plan2) {
+            double ang = -2.0 * M_PI * (double)j / (double)L;
+            tab[2 * j] = (float)std::cos(ang);
+            tab[2 * j + 1] = (float)std::sin(ang);
+        }
+        tab[2 * NR + j] = (float)w[j];
     }
     for (int i = 0; i < nE; ++i) {
         double x = E[i] / (kb_mev * temperature_K);
         double B = (x == 0.0) ? 1.0 : x / (-std::expm1(-x));
-        tab[3 * (size_t)L + i] = (float)(B / ((double)L * sw2 * (double)nchunks));
+        tab[2 * NR + (size_t)L + i] = (float)(B / ((double)L * sw2 * (double)nchunks));
     }
     int rc = ensure(ctx, (void**)&ctx->d_spec_tab, &ctx->spec_tab_bytes, sizeof(float) * tab.size());
     if (rc) return rc;
@@ -574,7 +582,7 @@ static int spectrum_core(tacaw_ctx* ctx, const void* d_buf, int nprobes, int64_t
     for (int c = 0; c < nchunks; ++c) {
         rc = launch_spectrum(ctx, (const float2*)d_buf + (size_t)c * step * (size_t)nroi, nprobes, nroi, L,
                              (size_t)nframes_total * (size_t)nroi, c > 0, (const float2*)ctx->d_spec_tab,
-                             ctx->d_spec_tab + 2 * (size_t)L, ctx->d_spec_tab + 3 * (size_t)L, e_lo, nE, d_I, st);
+                             ctx->d_spec_tab + 2 * NR, ctx->d_spec_tab + 2 * NR + (size_t)L, e_lo, nE, d_I, st);
         if (rc) return rc;
     }
     return TACAW_OK;

@@ -6,8 +6,10 @@
 // the multislice column kernel: thread (tid, c) holds frames tid + Tt*m of series r0+c, the
 // transform leaves it with bins tid + Tt*m, which it scales and stores.  The window and the
 // per-energy factor bose[e] = B(E_e/kBT)/(T sum w^2) are fp64-computed host tables.
+#include <cstdlib>
+
 #include "ctx.h"
-#include "fft_core.cuh"
+#include "fft2.cuh"
 
 namespace tacaw {
 
@@ -82,6 +84,89 @@ __global__ void __launch_bounds__(SpecCfg<N>::THREADS) k_spectrum(const float2* 
     }
 }
 
+// Series of 512 frames and more: the single-exchange transform of the slice-step kernels (fft2.cuh; thread (tid, c) holds the
+// 32 frames tid + Tt*m of series r0+c, one padded exchange, twiddles from the Plan2 table in shared memory).  Half the
+// shared memory of the ping-pong plan above and twice the loads in flight per thread.
+template <int N>
+struct SpecCfg2 {
+    using P = Plan2<N>;
+    static constexpr int E = P::E, T = P::T;
+    // series per CTA, measured on B200 for 32 x 7721 series (ms at 512 / 1024 / 2048 frames): 8: 0.69 / 1.52 / 3.37,
+    // 16: 0.63 / 1.60 / -, 4: - / - / 3.87; the two-exchange plan above: 0.75 / 1.83 / 4.28
+    static constexpr int WQ = (N == 512) ? 16 : 8;
+    static constexpr int THREADS = T * WQ;
+    static constexpr int XE = exch2_elems(N, WQ);
+    static constexpr size_t smem() { return sizeof(float2) * ((size_t)P::TW_ELEMS + XE); }
+};
+
+template <int N>
+__global__ void __launch_bounds__(SpecCfg2<N>::THREADS) k_spectrum2(const float2* __restrict__ buf, long long nroi,
+                                                                    size_t probe_stride, int accumulate,
+                                                                    const float2* __restrict__ table,
+                                                                    const float* __restrict__ window,
+                                                                    const float* __restrict__ bose, int e_lo, int nE,
+                                                                    float* __restrict__ I) {
+    using C = SpecCfg2<N>;
+    using P = Plan2<N>;
+    constexpr int E = C::E, T = C::T, WQ = C::WQ;
+    extern __shared__ __align__(16) float2 smem[];
+    const int lt = threadIdx.x;
+    const int c = lt % WQ, tid = lt / WQ;
+    float2* tw = smem;
+    float2* ex = smem + P::TW_ELEMS;
+    fft2_load_twiddles<N>(tw, table, lt, C::THREADS);
+    const int p = blockIdx.y;
+    const long long r = (long long)blockIdx.x * WQ + c;
+    const bool live = r < nroi;
+    const float2* src = buf + (size_t)p * probe_stride + (live ? r : 0);
+    float2 x[E];
+#pragma unroll
+    for (int m = 0; m < E; ++m) {
+        const int f = tid + T * m;
+        x[m] = live ? src[(size_t)f * nroi] : make_float2(0.f, 0.f);
+    }
+#pragma unroll
+    for (int m = 0; m < E; ++m) {
+        const float w = window[tid + T * m];
+        x[m] = make_float2(x[m].x * w, x[m].y * w);
+    }
+    cp_async_wait_all();
+    __syncthreads();                               // twiddle table complete
+    SyncBlock sync;
+    fft2<N, WQ, false, false>(x, tw + tid, ex, tid, c, sync);
+    if (!live) return;
+    float* dst = I + (size_t)p * nE * (size_t)nroi + r;
+#pragma unroll
+    for (int m = 0; m < E; ++m) {
+        const int kbin = tid + T * m;
+        const int e = ((kbin + N / 2) & (N - 1)) - e_lo;      // position on the ascending energy axis
+        if (e >= 0 && e < nE) {
+            const float v = bose[e] * (x[m].x * x[m].x + x[m].y * x[m].y);
+            dst[(size_t)e * nroi] = accumulate ? dst[(size_t)e * nroi] + v : v;
+        }
+    }
+}
+
+template <int N>
+static int launch_spec2_n(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int64_t nroi, size_t probe_stride, int accumulate,
+                          const float2* table, const float* d_window, const float* d_bose, int e_lo, int nE, float* d_I,
+                          cudaStream_t st) {
+    using C = SpecCfg2<N>;
+    const size_t smem = C::smem();
+    auto kern = k_spectrum2<N>;
+    if (smem > 48 * 1024) TACAW_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int64_t gx = (nroi + C::WQ - 1) / C::WQ;
+    for (int p0 = 0; p0 < nprobes; p0 += 32768) {
+        int np = nprobes - p0 < 32768 ? nprobes - p0 : 32768;
+        kern<<<dim3((unsigned)gx, np), C::THREADS, smem, st>>>(d_buf + (size_t)p0 * probe_stride, (long long)nroi, probe_stride, accumulate,
+                                                              table, d_window, d_bose, e_lo, nE,
+                                                              d_I + (size_t)p0 * nE * (size_t)nroi);
+        ctx->launches++;
+    }
+    TACAW_CUDA(ctx, cudaGetLastError());
+    return TACAW_OK;
+}
+
 template <int N>
 static int launch_spec_n(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int64_t nroi, size_t probe_stride, int accumulate,
                          const float2* roots,
@@ -153,6 +238,14 @@ int launch_detect(tacaw_ctx* ctx, const float* d_I, int nprobes, int nE, int64_t
 int launch_spectrum(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int64_t nroi, int nframes, size_t probe_stride,
                     int accumulate, const float2* d_roots,
                     const float* d_window, const float* d_bose, int e_lo, int nE, float* d_I, cudaStream_t st) {
+    static const bool two_exchange = [] { const char* e = getenv("TACAW_SPEC_TWO_EXCHANGE"); return e && atoi(e) != 0; }();
+    if (two_exchange) {       // comparison switch: the ping-pong plan for the long series too
+        switch (nframes) {
+            case 512: return launch_spec_n<512>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+            case 1024: return launch_spec_n<1024>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+            case 2048: return launch_spec_n<2048>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+        }
+    }
     switch (nframes) {
         case 8: return launch_spec_n<8>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
         case 16: return launch_spec_n<16>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
@@ -160,9 +253,9 @@ int launch_spectrum(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int64_t nr
         case 64: return launch_spec_n<64>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
         case 128: return launch_spec_n<128>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
         case 256: return launch_spec_n<256>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
-        case 512: return launch_spec_n<512>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
-        case 1024: return launch_spec_n<1024>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
-        case 2048: return launch_spec_n<2048>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+        case 512: return launch_spec2_n<512>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+        case 1024: return launch_spec2_n<1024>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+        case 2048: return launch_spec2_n<2048>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
     }
     return fail(ctx, TACAW_E_UNSUPPORTED, "nframes must be a power of two in [8, 2048]");
 }
