@@ -92,7 +92,7 @@ struct SpecCfg2 {
     using P = Plan2<N>;
     static constexpr int E = P::E, T = P::T;
     // series per CTA, measured on B200 for 32 x 7721 series (ms at 512 / 1024 / 2048 frames): 8: 0.69 / 1.52 / 3.37,
-    // 16: 0.63 / 1.60 / -, 4: - / - / 3.87; the two-exchange plan above: 0.75 / 1.83 / 4.28
+    // 16: 0.63 / 1.60 / -, 4: - / 1.95 / 3.87; the two-exchange plan above: 0.75 / 1.83 / 4.28
     static constexpr int WQ = (N == 512) ? 16 : 8;
     static constexpr int THREADS = T * WQ;
     static constexpr int XE = exch2_elems(N, WQ);
