@@ -148,6 +148,8 @@ int tacaw_accumulate(tacaw_ctx *ctx, const void *d_qwaves, int nwaves, const int
  *   I[p][e][r] = B(E_e/(k_B T_K)) |Phi|^2 / (T sum_f w_f^2),  B(x) = x/(1-exp(-x)), B(0) = 1
  * Energies ascending, restricted to [emin_meV, emax_meV] (inclusive, 1e-9 meV slack).
  * nframes: power of two in [8, 2048].
+ * Series of 512 frames and more run on the single-exchange transform of the slice-step kernels; the environment variable
+ * TACAW_SPEC_TWO_EXCHANGE=1 (read once) keeps the two-exchange plan of the shorter series for comparison -- same results.
  * d_I HOST-NULLABLE: pass d_I = NULL to query nE / the axis only.
  * d_I      DEVICE float [nprobes][nE][nroi];  E_axis_meV_out HOST double [>= nE] or NULL; nE HOST. */
 int tacaw_spectrum(tacaw_ctx *ctx, const void *d_buf, int nprobes, int64_t nroi, int nframes, double dt_fs,
