@@ -239,15 +239,54 @@ def window_table(kind: str, n: int, param: float = 0.0) -> np.ndarray:
     if kind == "kaiser":
         u = 2 * x - 1
         return np.i0(param * np.sqrt(np.maximum(0.0, 1 - u * u))) / np.i0(param)
+    if kind == "dolph_chebyshev":
+        return dolph_chebyshev(n, float(param))
     raise ValueError(kind)
 
 
-def chunk_starts(nframes_total: int, chunk_len: int, chunk_overlap: int):
+def dolph_chebyshev(n: int, attenuation_db: float) -> np.ndarray:
+    """'the Dolph-Chebyshev window with attenuation 100 dB' (Appendix A; the paper points to scipy [59] for
+    the definition).  Definition written out: the window of M points whose discrete-time Fourier transform is the
+    Chebyshev polynomial of order M-1 in x0 cos(theta/2), all side lobes `attenuation_db` below the main lobe:
+        W(theta) = T_{M-1}(x0 cos(theta/2)),   x0 = cosh(acosh(10^(att/20)) / (M-1)),
+        w[j] = (1/M) sum_{k=0}^{M-1} W(2 pi k/M) cos(2 pi k (j - (M-1)/2) / M),   normalised to max w = 1
+    (the sum is the inverse DFT of the M samples of W, centred on the window's midpoint; T_m(x) = cos(m acos x) for
+    |x| <= 1, cosh(m acosh x) for x > 1, (-1)^m cosh(m acosh(-x)) for x < -1).  Periodic form (reading G9): the symmetric
+    window of M = n + 1 points without its last sample.  Plain O(M^2) loops, no FFT."""
+    M = n + 1
+    if M < 2:
+        return np.ones(n)
+    m = M - 1
+    x0 = np.cosh(np.arccosh(10.0 ** (abs(attenuation_db) / 20.0)) / m)
+
+    def cheb(x: float) -> float:
+        if x > 1.0:
+            return float(np.cosh(m * np.arccosh(x)))
+        if x < -1.0:
+            return float((1.0 if m % 2 == 0 else -1.0) * np.cosh(m * np.arccosh(-x)))
+        return float(np.cos(m * np.arccos(x)))
+
+    W = np.array([cheb(x0 * np.cos(np.pi * k / M)) for k in range(M)])      # W(theta_k), theta_k = 2 pi k / M
+    w = np.zeros(M)
+    for j in range(M):
+        acc = 0.0
+        for k in range(M):
+            acc += W[k] * np.cos(2.0 * np.pi * k * (j - 0.5 * m) / M)
+        w[j] = acc / M
+    w = w / w.max()
+    return w[:n].copy()
+
+
+def chunk_starts(nframes_total: int, chunk_len: int, chunk_overlap: int, skip_init: int = 0, stride: int = 1):
     """'If a chunk indexed by n starts at snapshot s_n, then the next chunk starts at
-    s_{n+1} = s_n + L/nu, using remainder-less division'; only complete chunks are used."""
-    step = chunk_len // chunk_overlap
-    out, s = [], 0
-    while s + chunk_len <= nframes_total:
+    s_{n+1} = s_n + L/nu, using remainder-less division'; only complete chunks are used.
+    skip_init: the first `skip_init` snapshots are discarded (Listing 1 :443 `trajectory_chunks_skip_init = 200`: the
+    3 ps thermalisation period of :164 at 15 fs).  stride: 'a stride for snapshot reading' (:140) -- chunk n holds the L
+    snapshots s_n, s_n + stride, ..., and s counts in units of the stored snapshots, so the next chunk starts
+    (L/nu) * stride stored snapshots later (reading G24)."""
+    step = (chunk_len // chunk_overlap) * stride
+    out, s = [], skip_init
+    while s + (chunk_len - 1) * stride + 1 <= nframes_total:
         out.append(s)
         s += step
     return out
@@ -272,16 +311,18 @@ def spectrum_table(buf: np.ndarray, frame0: int, nframes: int, dt_fs: float, w: 
 
 
 def spectrum_welch(buf: np.ndarray, chunk_len: int, chunk_overlap: int, dt_fs: float, w: np.ndarray, temperature_K: float,
-                   emin: float = -np.inf, emax: float = np.inf):
+                   emin: float = -np.inf, emax: float = np.inf, skip_init: int = 0, stride: int = 1):
     """Eq.(2): the average over the N trajectory chunks of I_i(q,E), each chunk windowed, transformed,
-    squared and Bose-corrected as in O9 (:142).  Returns (I [P][nE][Q], E [nE], N)."""
-    starts = chunk_starts(buf.shape[1], chunk_len, chunk_overlap)
+    squared and Bose-corrected as in O9 (:142).  With a snapshot stride the chunk's time step is stride * dt.
+    Returns (I [P][nE][Q], E [nE], N)."""
+    starts = chunk_starts(buf.shape[1], chunk_len, chunk_overlap, skip_init, stride)
     acc, E = None, None
     for s in starts:
-        I, E = spectrum_table(buf, s, chunk_len, dt_fs, w, temperature_K, emin, emax)
+        sub = np.ascontiguousarray(buf[:, s: s + (chunk_len - 1) * stride + 1: stride])     # the chunk's L snapshots
+        I, E = spectrum_table(sub, 0, chunk_len, dt_fs * stride, w, temperature_K, emin, emax)
         acc = I / len(starts) if acc is None else acc + I / len(starts)
     if E is None:
-        E, _ = energy_axis(chunk_len, dt_fs, emin, emax)
+        E, _ = energy_axis(chunk_len, dt_fs * stride, emin, emax)
     return acc, E, len(starts)
 
 

@@ -55,3 +55,29 @@ def run(wl, probes: Optional[Sequence[int]] = None, pot_mode: int = 1) -> Dict[s
     emin, emax = wl.e_roi_meV if wl.e_roi_meV is not None else (-np.inf, np.inf)
     I, E = spectrum(buf, wl.dt_fs, wl.window, wl.temperature_K, emin, emax)
     return dict(I=I, E=E, roi=roi, buf=buf)
+
+
+def run_reassembled(wl, offsets: np.ndarray, chunk_len: int, probes: Optional[Sequence[int]] = None,
+                    pot_mode: int = 1) -> np.ndarray:
+    """'one may perform a single longer MD trajectory and, for each averaging chunk in the TACAW
+    calculation, construct the stacked supercell from randomly selected segments of that trajectory.'
+    The workload's z-segments all follow segment 0's trajectory; for chunk i, stack position k shows that trajectory from
+    snapshot offsets[i][k] on, so chunk frame f is built from trajectory frames offsets[i][k] + f (the offsets are drawn
+    by the seeded input generator, never here).  Returns the time-ordered buffers [nchunks][P][chunk_len][Q] (c128)."""
+    pr = list(range(wl.nprobes)) if probes is None else list(probes)
+    roi = roi_for(wl)
+    nch, nstack = offsets.shape
+    seg = wl.segments[0]
+    psi0 = make_probes(wl.nx, wl.ny, wl.lx, wl.ly, wl.lam, wl.probes_xy[pr], wl.alpha_mrad * 1e-3)
+    out = np.zeros((nch, len(pr), chunk_len, roi.size), dtype=np.complex128)
+    for i in range(nch):
+        for f in range(chunk_len):
+            tr = []
+            for k in range(nstack):
+                t = int(offsets[i, k]) + f
+                pos = seg.frames(t, t + 1, wl.dt_fs)[0]
+                tr.append(build_slices(wl.nx, wl.ny, wl.lx, wl.ly, pos, seg.species, wl.a, wl.b, wl.dz, seg.nslices, 0.0,
+                                       wl.sigma, bandlimit=wl.bandlimit, pot_mode=pot_mode)["trans"])
+            q = propagate(wl.lx, wl.ly, wl.lam, wl.bandlimit, psi0, None, [tr], wl.dz, 1)
+            accumulate(q, np.arange(len(pr)), np.full(len(pr), f), roi, out[i])
+    return out

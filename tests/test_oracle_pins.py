@@ -45,6 +45,18 @@ def test_p8_fft_vs_naive_vs_numpy(oracle, n):
             assert np.linalg.norm(oracle.dft_naive(x, sign) - ref) <= 1e-13 * scale
 
 
+@pytest.mark.parametrize("n", [200, 1680])
+def test_p8_naive_dft_at_the_papers_non_power_of_two_lengths(oracle, n):
+    """The paper's chunk length 200 (:164) and grid edge 1680 = 2^4 3 5 7 (:162): the oracle's dispatch falls back to
+    its naive DFT for such lengths; pinned against numpy.fft (library routine, test only)."""
+    rng = np.random.default_rng(n)
+    x = rng.normal(size=n) + 1j * rng.normal(size=n)
+    for sign, ref in ((-1, np.fft.fft(x)), (+1, np.fft.ifft(x) * n)):
+        assert np.max(np.abs(oracle.dft_naive(x, sign) - ref)) <= 1e-10 * np.max(np.abs(ref))
+    a = rng.normal(size=(3, n)) + 1j * rng.normal(size=(3, n))
+    assert np.max(np.abs(oracle.fft2(a, -1) - np.fft.fft2(a))) <= 1e-10 * np.max(np.abs(a)) * n
+
+
 @pytest.mark.parametrize("shape", [(8, 8), (16, 64), (128, 32), (256, 256)])
 def test_p8_fft2_vs_numpy(oracle, shape):
     rng = np.random.default_rng(5)

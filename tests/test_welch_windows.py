@@ -1,6 +1,8 @@
 """Welch chunk averaging (Eq.(2) :126) and the further window
 functions (:170-182).  Pins of the oracle against scipy's library routines and closed forms (CPU), the host window
 generator of the library against the oracle (CPU, no GPU compute), and GPU parity of tacaw_spectrum_welch."""
+import os
+
 import numpy as np
 import pytest
 
@@ -58,6 +60,68 @@ def test_w4_chunk_starts_follow_the_paper_rule(oracle):
     assert oracle.chunk_starts(16, 16, 2) == [0]
     assert oracle.chunk_starts(15, 16, 2) == []
     assert oracle.chunk_starts(1024 + 512, 1024, 1) == [0]
+
+
+def golden():
+    out = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "paper_worked_numbers.txt")) as fh:
+        for line in fh:
+            if line.startswith("#") or "|" not in line:
+                continue
+            k, v, _ = [t.strip() for t in line.split("|", 2)]
+            out[k] = v
+    return out
+
+
+def test_w4b_the_papers_31_chunks(oracle):
+    """a 51 ps trajectory stored every 15 fs (3400 snapshots), the first 3 ps (200 snapshots, Listing 1
+    :443 trajectory_chunks_skip_init) discarded, chunks of 200 with nu = 2 -> 'an average over 31 chunks'."""
+    g = golden()
+    nsnap = round(51e3 / 15.0)
+    skip = int(g["welch_skip_init_listing1"])
+    assert skip == round(3e3 / 15.0)
+    st = oracle.chunk_starts(nsnap, 200, 2, skip_init=skip)
+    assert len(st) == int(g["welch_chunks_51ps_minus_3ps_15fs_L200_nu2"])
+    assert st[0] == skip and st[1] - st[0] == 100 and st[-1] + 200 == nsnap
+    # the same 48 ps without the thermalisation period in the file
+    assert len(oracle.chunk_starts(nsnap - skip, 200, 2)) == 31
+
+
+def test_w4c_stride_and_skip(oracle):
+    """Snapshot stride (:140): chunk n holds snapshots s_n, s_n + stride, ...; complete chunks only."""
+    assert oracle.chunk_starts(40, 8, 2, skip_init=3, stride=2) == [3, 11, 19]          # 3 + 7*2 = 17 <= 39, ..., 19 + 14 = 33; 27 + 14 = 41 > 39
+    assert oracle.chunk_starts(40, 8, 2, stride=1) == oracle.chunk_starts(40, 8, 2)
+    assert oracle.chunk_starts(16, 8, 1, stride=2) == [0]
+    assert oracle.chunk_starts(15, 8, 1, stride=2) == [0]
+    assert oracle.chunk_starts(14, 8, 1, stride=2) == []
+    # a strided Welch average equals the plain one on the decimated series with time step stride*dt
+    rng = np.random.default_rng(11)
+    buf = series(rng, 2, 48, 3)
+    w = oracle.window_table("hann", 8)
+    I1, E1, n1 = oracle.spectrum_welch(buf, 8, 2, 5.0, w, 300.0, skip_init=4, stride=3)
+    I2, E2, n2 = oracle.spectrum_welch(np.ascontiguousarray(buf[:, 4::3]), 8, 2, 15.0, w, 300.0)
+    # decimated series: starts every 4 decimated snapshots = 12 stored ones, same as (L/nu)*stride
+    assert n1 == n2 and np.array_equal(E1, E2) and np.max(np.abs(I1 - I2)) <= 1e-14 * np.max(I2)
+
+
+def test_w8_dolph_chebyshev_100dB(oracle):
+    """PAPER.md:352: 'the Dolph-Chebyshev window with attenuation 100 dB ... See scipy and its documentation'.
+    (a) against scipy.signal.windows.chebwin in its periodic form; (b) the defining property, checked without scipy:
+    every side lobe of the symmetric window's transform sits 100 dB below the main lobe (equiripple)."""
+    import scipy.signal.windows as sw
+    att = float(golden()["chebwin_attenuation_dB"])
+    for n in (16, 17, 200, 256, 1024):
+        assert np.max(np.abs(oracle.window_table("dolph_chebyshev", n, att) - sw.chebwin(n, at=att, sym=False))) <= 2e-13
+    M = 65
+    w = np.append(oracle.dolph_chebyshev(M - 1, att), 0.0)
+    w[-1] = w[0]                                              # symmetric window of M points (periodic form + last sample)
+    Wf = np.abs(np.fft.fft(w, 64 * M))
+    Wf /= Wf[0]
+    # main-lobe edge: first point where the response has fallen to the ripple level
+    lvl = 10.0 ** (-att / 20.0)
+    first = int(np.argmax(Wf < lvl * 1.0001))
+    side = Wf[first: Wf.size - first]
+    assert side.max() <= lvl * 1.001 and side.max() >= lvl * 0.98      # equiripple at exactly -100 dB
 
 
 def test_w5_single_chunk_is_the_plain_spectrum(oracle):
