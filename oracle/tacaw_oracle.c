@@ -146,14 +146,25 @@ void oracle_fft1d(int n, double *x, int sign) {
  * sign=-1 forward (no scaling); sign=+1 inverse (scaled by 1/(nx ny)). */
 void oracle_fft2(int ny, int nx, double *a, int sign) {
     int nmax = nx > ny ? nx : ny;
-    double *tmp = (double *)malloc(sizeof(double) * 4 * (size_t)nmax);
-    for (int iy = 0; iy < ny; ++iy) fft1d_strided(nx, a + 2 * (size_t)iy * nx, 1, sign, tmp, tmp + 2 * nmax);
-    for (int ix = 0; ix < nx; ++ix) fft1d_strided(ny, a + 2 * (size_t)ix, nx, sign, tmp, tmp + 2 * nmax);
+    /* rows, then columns: independent 1D transforms, shared out over threads when the caller is not already
+     * running in parallel (the arithmetic of each transform is untouched) */
+    int par = 1;
+#ifdef _OPENMP
+    par = !omp_in_parallel() && (size_t)nx * ny >= 65536;
+#endif
+#pragma omp parallel if (par)
+    {
+        double *tmp = (double *)malloc(sizeof(double) * 4 * (size_t)nmax);
+#pragma omp for schedule(static)
+        for (int iy = 0; iy < ny; ++iy) fft1d_strided(nx, a + 2 * (size_t)iy * nx, 1, sign, tmp, tmp + 2 * nmax);
+#pragma omp for schedule(static)
+        for (int ix = 0; ix < nx; ++ix) fft1d_strided(ny, a + 2 * (size_t)ix, nx, sign, tmp, tmp + 2 * nmax);
+        free(tmp);
+    }
     if (sign > 0) {
         double s = 1.0 / ((double)nx * (double)ny);
         for (size_t i = 0; i < 2 * (size_t)nx * ny; ++i) a[i] *= s;
     }
-    free(tmp);
 }
 
 /* O5 mask: M[h,k] = 1 iff q^2 <= (2/3)^2 min(Nx/(2Lx), Ny/(2Ly))^2.  For a square cell this is
@@ -316,7 +327,13 @@ int oracle_propagate(int nx, int ny, double lx, double ly, double lambda, int ba
         }
     }
     int bad = 0;
-#pragma omp parallel for schedule(dynamic, 1)
+    /* waves are independent: one thread per wave when there are enough of them, otherwise the waves run one after
+     * the other and each 2D transform is shared out over the threads instead (oracle_fft2) */
+    int over_waves = 1;
+#ifdef _OPENMP
+    over_waves = nwaves >= omp_get_max_threads();
+#endif
+#pragma omp parallel for schedule(dynamic, 1) if (over_waves)
     for (int w = 0; w < nwaves; ++w) {
         double *psi = waves + 2 * npix * w;
         int f = wave_frame ? wave_frame[w] : 0;
