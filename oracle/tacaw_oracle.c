@@ -202,6 +202,25 @@ int oracle_build_slices(int nx, int ny, double lx, double ly, const double *pos,
     }
     if (n_clamped) *n_clamped = clamped;
     size_t npix = (size_t)nx * ny;
+    /* f_s(q^2) depends on the species and the pixel only, not on the atom: evaluated once per (species, pixel) with the
+     * same expression and used for every atom of that species below (a table of the values, no change of arithmetic) */
+    double *ftab = (double *)calloc((size_t)(nspecies > 0 ? nspecies : 1) * npix, sizeof(double));
+    unsigned char *carries = (unsigned char *)calloc(npix, 1);   /* 1 where V is defined: in band, not on a Nyquist line */
+#pragma omp parallel for schedule(static)
+    for (int iy = 0; iy < ny; ++iy) {
+        int k = signed_index(iy, ny);
+        for (int ix = 0; ix < nx; ++ix) {
+            int h = signed_index(ix, nx);
+            carries[(size_t)iy * nx + ix] = (2 * k != -ny) && (2 * h != -nx) && in_band(h, k, nx, ny, lx, ly, bandlimit);
+            double q2 = (h / lx) * (h / lx) + (k / ly) * (k / ly);
+            for (int sidx = 0; sidx < nspecies; ++sidx) {
+                const double *as = a + 4 * sidx, *bs = b + 4 * sidx;
+                double f = 0.0;
+                for (int i = 0; i < 4; ++i) f += as[i] * exp(-bs[i] * q2);
+                ftab[(size_t)sidx * npix + (size_t)iy * nx + ix] = f;
+            }
+        }
+    }
     double worst_ratio = 0.0;
 #pragma omp parallel for schedule(dynamic, 1) reduction(max : worst_ratio)
     for (int n = 0; n < nslices; ++n) {
@@ -210,7 +229,7 @@ int oracle_build_slices(int nx, int ny, double lx, double ly, const double *pos,
         double *ey = (double *)malloc(sizeof(double) * 2 * (size_t)ny);
         for (int j = 0; j < natoms; ++j) {
             if (slice_of[j] != n) continue;
-            const double *as = a + 4 * species[j], *bs = b + 4 * species[j];
+            const double *fs = ftab + (size_t)species[j] * npix;
             double xf = pos[3 * j] / lx, yf = pos[3 * j + 1] / ly;
             if (pot_mode == 1) {
                 for (int ix = 0; ix < nx; ++ix) {
@@ -224,14 +243,10 @@ int oracle_build_slices(int nx, int ny, double lx, double ly, const double *pos,
             }
             for (int iy = 0; iy < ny; ++iy) {
                 int k = signed_index(iy, ny);
-                if (2 * k == -ny) continue;                      /* Nyquist never carries V */
                 for (int ix = 0; ix < nx; ++ix) {
                     int h = signed_index(ix, nx);
-                    if (2 * h == -nx) continue;
-                    if (!in_band(h, k, nx, ny, lx, ly, bandlimit)) continue;
-                    double q2 = (h / lx) * (h / lx) + (k / ly) * (k / ly);
-                    double f = 0.0;
-                    for (int i = 0; i < 4; ++i) f += as[i] * exp(-bs[i] * q2);
+                    if (!carries[(size_t)iy * nx + ix]) continue;   /* Nyquist lines and out-of-band pixels carry no V */
+                    double f = fs[(size_t)iy * nx + ix];
                     double pr, pi_;
                     if (pot_mode == 1) {
                         pr = ex[2 * ix] * ey[2 * iy] - ex[2 * ix + 1] * ey[2 * iy + 1];
@@ -265,6 +280,8 @@ int oracle_build_slices(int nx, int ny, double lx, double ly, const double *pos,
     }
     if (max_imag) *max_imag = worst_ratio;
     free(slice_of);
+    free(ftab);
+    free(carries);
     return 0;
 }
 
