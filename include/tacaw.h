@@ -13,9 +13,18 @@
  *     1/Angstrom (no 2 pi).  Forward transform uses exp(-2 pi i ...); inverse carries 1/(nx ny).
  *   - nx, ny: powers of two in [16, 2048] (they may differ).
  *   - Every "d_" pointer is DEVICE memory owned by the caller; the library never frees or
- *     reallocates it.  The library owns only the context (tables and a small scratch buffer).
+ *     reallocates it.  The library owns only the context (twiddle / propagator tables, a pinned host
+ *     arena for index uploads, streams and events) -- all created in tacaw_create.  Scratch for the
+ *     calls is ONE caller-owned device buffer (tacaw_workspace_bytes / tacaw_set_workspace): no call
+ *     allocates, frees or device-synchronises.  A call whose scratch does not fit returns TACAW_E_NOMEM.
  *   - `stream` is a cudaStream_t cast to void* (NULL = default stream).  Calls enqueue work on it
  *     and return without synchronising unless stated; host outputs are written before return.
+ *   - ONE STREAM AT A TIME PER CONTEXT: consecutive calls on a context must be issued on the same stream, or be
+ *     ordered by the caller (event / synchronise) when the stream changes -- the workspace regions and the
+ *     propagator tables are reused in stream order.  To overlap, e.g., tacaw_build_slices of the next frame block
+ *     with tacaw_propagate of the current one, use two contexts (each with its own workspace).
+ *   - Every entry point makes the context's device current for the duration of the call and restores the caller's
+ *     current device before returning.
  *   - Every call returns TACAW_OK (0) or a negative TACAW_E_* code; nothing throws or exits.
  *     tacaw_last_error(ctx) gives a message for the last failure on that context.
  *   - There is no CPU fallback: without a CUDA device tacaw_create fails with TACAW_E_CUDA.
@@ -33,7 +42,7 @@ extern "C" {
 #define TACAW_OK 0
 #define TACAW_E_ARG (-1)         /* bad argument (null pointer, negative size, index out of range) */
 #define TACAW_E_UNSUPPORTED (-2) /* grid or series length outside the supported set */
-#define TACAW_E_NOMEM (-3)       /* scratch allocation failed */
+#define TACAW_E_NOMEM (-3)       /* the caller's workspace is missing or too small for this call */
 #define TACAW_E_CUDA (-4)        /* CUDA runtime error (message in tacaw_last_error) */
 
 typedef struct tacaw_ctx tacaw_ctx;
@@ -67,6 +76,9 @@ typedef struct {
 #define TACAW_WINDOW_TUKEY 2            /* param = alpha in [0,1]: cosine tapers of total fractional width alpha; 1 = Hann, 0 = rect (:170) */
 #define TACAW_WINDOW_BLACKMAN_HARRIS 3  /* 4-term, 0.35875 - 0.48829 cos(2 pi x) + 0.14128 cos(4 pi x) - 0.01168 cos(6 pi x) */
 #define TACAW_WINDOW_KAISER 4           /* param = beta >= 0: I0(beta sqrt(1 - (2x-1)^2)) / I0(beta) */
+#define TACAW_WINDOW_DOLPH_CHEBYSHEV 5  /* param = side-lobe attenuation in dB > 0 (the paper uses 100 dB, :352): the window whose
+                                           transform is the Chebyshev polynomial T_n(x0 cos(theta/2)), x0 = cosh(acosh(10^(dB/20))/n),
+                                           i.e. every side lobe `param` dB below the main lobe; max = 1 */
 
 /* Library version string and the SM architecture it was compiled for ("sm_100a"). */
 const char *tacaw_version(void);
@@ -76,6 +88,29 @@ const char *tacaw_version(void);
 int tacaw_create(tacaw_ctx **ctx, const tacaw_grid *grid, const tacaw_beam *beam, int device);
 int tacaw_destroy(tacaw_ctx *ctx);
 const char *tacaw_last_error(const tacaw_ctx *ctx);
+
+/* Workspace ("every device buffer is allocated by the caller").  tacaw_sizes announces the LARGEST
+ * call of each kind the caller will make; tacaw_workspace_bytes returns the bytes those calls need in total (each entry
+ * point gets its own 256-byte aligned region, so no two entry points share scratch); tacaw_set_workspace hands the
+ * library a device buffer of at least that size (256-byte aligned; it stays the caller's and must outlive every call
+ * queued against it).  It may be called again with a larger buffer once the work queued on the old one is ordered
+ * before the next call (same stream).  Calls that need no scratch (tacaw_detect, the HOST helpers) work without one. */
+typedef struct {
+    int natoms;       /* atoms per tacaw_build_slices call (one z-segment) */
+    int nframes;      /* frames per tacaw_build_slices call and frames in flight per tacaw_propagate call */
+    int nslices;      /* slices per tacaw_build_slices call (largest segment) */
+    int nsegments;    /* z-segments per tacaw_propagate call (0 = 1) */
+    int nwaves;       /* waves per tacaw_propagate / tacaw_accumulate call */
+    int nprobes;      /* probes per tacaw_make_probes call */
+    int host_staging; /* 1: also reserve the staging region of tacaw_build_slices_host (natoms x nframes positions) */
+} tacaw_sizes;
+size_t tacaw_workspace_bytes(const tacaw_ctx *ctx, const tacaw_sizes *sizes);
+int tacaw_set_workspace(tacaw_ctx *ctx, void *d_workspace, size_t bytes, const tacaw_sizes *sizes);
+
+/* Device-side error flags raised by kernels since the last check (at present: a species id outside
+ * [0, nspecies) seen by tacaw_build_slices, which then uses species 0 for that atom).  Synchronises `stream`,
+ * returns TACAW_E_ARG and clears the flags if any was raised, TACAW_OK otherwise. */
+int tacaw_device_status(tacaw_ctx *ctx, void *stream);
 
 /* Number of kernels this context has launched since creation (bench.py's gpu_launches). */
 int64_t tacaw_launch_count(const tacaw_ctx *ctx);
@@ -91,7 +126,8 @@ int64_t tacaw_launch_count(const tacaw_ctx *ctx);
  * d_species DEVICE int32 [natoms] in [0,nspecies), nspecies <= 8
  * d_trans   DEVICE complex64 [nframes][nslices][ny][nx], written
  * n_clamped HOST, optional (total over the frames); when non-NULL the call synchronises the stream
- *           before returning. */
+ *           before returning and also returns TACAW_E_ARG if a species id was out of range (with NULL
+ *           that error is sticky on the device and reported by tacaw_device_status). */
 int tacaw_build_slices(tacaw_ctx *ctx, const double *d_pos_A, const int32_t *d_species, int natoms, int nframes,
                        const tacaw_species *species, double slice_thickness_A, int nslices, double z0_A,
                        void *d_trans, int *n_clamped, void *stream);
@@ -107,21 +143,22 @@ int tacaw_make_probes(tacaw_ctx *ctx, const double *probe_xy_A, int nprobes, dou
  *   psi <- IFFT2{ P M FFT2{ t_n psi } }  for all slices of segment 0, then segment 1, ...
  *   P[h,k] = exp(-i pi lambda dz q^2),  M = band-limit mask of the context.
  * d_waves     DEVICE complex64 [nwaves][ny][nx], overwritten with the exit waves.
- * d_probes    DEVICE complex64 [.][ny][nx] or NULL.  NULL: d_waves holds the entrance waves.
+ * d_probes    DEVICE complex64 [nprobes][ny][nx] or NULL.  NULL: d_waves holds the entrance waves.
  *             Non-NULL: wave w starts from d_probes[wave_probe[w]] (d_waves is output only).
- * wave_probe  HOST int32 [nwaves] (ignored when d_probes is NULL)
+ * wave_probe  HOST int32 [nwaves], values in [0, nprobes) (ignored when d_probes is NULL)
  * wave_frame  HOST int32 [nwaves], values in [0, nframes_in_flight); waves that share a frame
  *             should be adjacent (they then share each t_n read).
  * d_trans     HOST array [nframes_in_flight*nsegments] of DEVICE pointers;
  *             d_trans[f*nsegments+k] -> complex64 [nslices_per_segment[k]][ny][nx]
  * output_space 0: r-space psi_S;  1: q-space Psi_S = FFT2(psi_S), unnormalised, native FFT order. */
 /* Tuning knobs of tacaw_propagate, read from the environment (defaults swept on B200):
- *   TACAW_STREAMS=n        wave groups in flight, caller's stream + n-1 internal ones (default 3, max 4; read once)
- *   TACAW_L2_GROUP_MB=x    bytes of full waves per group (default L2/5, whole row tuples, at least 3 waves)
+ *   TACAW_STREAMS=n        wave groups in flight, caller's stream + n-1 internal ones (default 3, 2 for waves above the group
+ *                          budget, i.e. 2048^2; max 4; read once)
+ *   TACAW_L2_GROUP_MB=x    bytes of full waves per group (default L2/5, whole row tuples, at least 3 waves; 2 waves at 2048^2)
  *   TACAW_GRID_FRAC=f      fraction of the machine-filling grid a slice-step launch uses (default 1; 0.5-1 measured equal)
  *   TACAW_PDL=0            launch the slice-step kernels without programmatic dependent launch
  * They change scheduling only, never results (tests/test_gpu_parity.py::test_propagate_l2_grouping_is_transparent). */
-int tacaw_propagate(tacaw_ctx *ctx, void *d_waves, const void *d_probes, const int32_t *wave_probe,
+int tacaw_propagate(tacaw_ctx *ctx, void *d_waves, const void *d_probes, int nprobes, const int32_t *wave_probe,
                     const int32_t *wave_frame, int nwaves, const void *const *d_trans,
                     int nframes_in_flight, const int32_t *nslices_per_segment, int nsegments,
                     double slice_thickness_A, int output_space, void *stream);
@@ -162,17 +199,21 @@ int tacaw_spectrum(tacaw_ctx *ctx, const void *d_buf, int nprobes, int64_t nroi,
 int tacaw_make_window(int kind, int n, double param, double *w_out);
 
 /* Welch method over trajectory chunks (Eq.(2) :126):
- * the time-ordered buffer holds nframes_total frames; chunk n covers frames s_n .. s_n + L - 1 with
- * s_0 = 0, s_{n+1} = s_n + L/nu (remainder-less division), for every n with s_n + L <= nframes_total (N chunks);
+ * the time-ordered buffer holds nframes_total stored frames.  Chunk n holds the L frames s_n + f*frame_stride,
+ * f = 0..L-1 ("a stride for snapshot reading", :140), with s_0 = skip_init (Listing 1 :443
+ * trajectory_chunks_skip_init: snapshots discarded as thermalisation, :164) and s_{n+1} = s_n + (L/nu)*frame_stride
+ * (:138, remainder-less division, counted in the chunk's own snapshots; reading G24), for every n whose last frame
+ * exists (N complete chunks):
  *   I[p][e][r] = (1/N) sum_n B(E_e/(k_B T_K)) |Phi_n|^2 / (L sum_f w_f^2),  Phi_n = DFT over the chunk of w_f buf
- * with E_k = h k'/(L dt).  L = chunk_len: power of two in [8, 2048]; nu = chunk_overlap >= 1.
+ * with E_k = h k'/(L dt frame_stride).  L = chunk_len: power of two in [8, 2048]; nu = chunk_overlap >= 1;
+ * skip_init >= 0; frame_stride >= 1.  All chunks run in ONE launch (|Phi_n|^2 summed in registers, I written once).
  * window_table HOST double [L] (tacaw_make_window or the caller's own).  N = 0 (buffer shorter than a chunk)
  * leaves d_I untouched.  nchunks HOST out (may be NULL).  Other arguments as tacaw_spectrum;
  * d_buf DEVICE complex64 [nprobes][nframes_total][nroi], d_I DEVICE float [nprobes][nE][nroi]. */
 int tacaw_spectrum_welch(tacaw_ctx *ctx, const void *d_buf, int nprobes, int64_t nroi, int nframes_total, int chunk_len,
-                         int chunk_overlap, double dt_fs, const double *window_table, double temperature_K,
-                         double emin_meV, double emax_meV, float *d_I, double *E_axis_meV_out, int *nE, int *nchunks,
-                         void *stream);
+                         int chunk_overlap, int skip_init, int frame_stride, double dt_fs, const double *window_table,
+                         double temperature_K, double emin_meV, double emax_meV, float *d_I, double *E_axis_meV_out, int *nE,
+                         int *nchunks, void *stream);
 
 /* DetectorSet (PAPER.md:114 "circular and annular -- with arbitrary center and radii -- and custom", :148-150, :257;
  * SURVEY.md 8(f) item 2).  Two calls:
@@ -218,8 +259,10 @@ int tacaw_scan_batch(const int32_t *shape, const int32_t *batch_shape, int batch
                      int32_t *nbatches);
 
 /* Convenience for host-resident data (bench.py's end-to-end leg): same as the calls above but the
- * named buffers are HOST memory; the library stages them through its own device scratch with
- * cudaMemcpyAsync on `stream` and synchronises before returning. */
+ * named buffers are HOST memory; the library stages them through the staging region of the caller's workspace
+ * (tacaw_sizes.host_staging = 1) with cudaMemcpyAsync on `stream`.  Species ids are validated on the host
+ * (TACAW_E_ARG).  With n_clamped == NULL the call does not synchronise: the host arrays must then stay valid until
+ * the stream has consumed them (pinned memory; pageable memory is staged by the CUDA runtime before it returns). */
 int tacaw_build_slices_host(tacaw_ctx *ctx, const double *h_pos_A, const int32_t *h_species, int natoms, int nframes,
                             const tacaw_species *species, double slice_thickness_A, int nslices, double z0_A,
                             void *d_trans, int *n_clamped, void *stream);

@@ -16,6 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libtacaw.so")
 
 EXPORTS = ["tacaw_version", "tacaw_create", "tacaw_destroy", "tacaw_last_error", "tacaw_launch_count",
+           "tacaw_workspace_bytes", "tacaw_set_workspace", "tacaw_device_status",
            "tacaw_build_slices", "tacaw_build_slices_host", "tacaw_make_probes", "tacaw_propagate",
            "tacaw_make_roi", "tacaw_accumulate", "tacaw_spectrum", "tacaw_make_window", "tacaw_spectrum_welch",
            "tacaw_make_detector", "tacaw_detect", "tacaw_make_scan", "tacaw_scan_batch"]
@@ -24,7 +25,7 @@ DETECTORS = {"circular": 0, "annular": 1}
 
 SCAN_MODES = {"box": 0, "box_relative": 1, "unitcell": 2, "parallelogram": 3}
 
-WINDOWS = {"rect": 0, "hann": 1, "tukey": 2, "blackman_harris": 3, "kaiser": 4}
+WINDOWS = {"rect": 0, "hann": 1, "tukey": 2, "blackman_harris": 3, "kaiser": 4, "dolph_chebyshev": 5}
 
 ROI_MODES = {"full": 0, "disc": 1, "annulus": 2, "rect": 3}
 
@@ -45,6 +46,13 @@ class _Species(C.Structure):
     _fields_ = [("nspecies", C.c_int), ("a", C.c_void_p), ("b", C.c_void_p)]
 
 
+class _Sizes(C.Structure):
+    _fields_ = [("natoms", C.c_int), ("nframes", C.c_int), ("nslices", C.c_int), ("nsegments", C.c_int),
+                ("nwaves", C.c_int), ("nprobes", C.c_int), ("host_staging", C.c_int)]
+
+SIZE_KEYS = ("natoms", "nframes", "nslices", "nsegments", "nwaves", "nprobes", "host_staging")
+
+
 _lib = None
 
 
@@ -61,6 +69,8 @@ def load_library():
         lib.tacaw_last_error.argtypes = [C.c_void_p]
         lib.tacaw_launch_count.restype = C.c_int64
         lib.tacaw_launch_count.argtypes = [C.c_void_p]
+        lib.tacaw_workspace_bytes.restype = C.c_size_t
+        lib.tacaw_workspace_bytes.argtypes = [C.c_void_p, C.c_void_p]
         _lib = lib
     return _lib
 
@@ -103,6 +113,41 @@ class Tacaw:
         rc = self.lib.tacaw_create(C.byref(self._ctx), C.byref(g), C.byref(b), C.c_int(device))
         if rc != 0:
             raise TacawError(f"tacaw_create failed ({rc})")
+        self._ws = None                                  # the caller-owned workspace tensor (torch owns the memory)
+        self._ws_sizes = dict.fromkeys(SIZE_KEYS, 0)
+
+    # ------------------------------------------------------------------------------------------
+    def workspace_bytes(self, **sizes) -> int:
+        """tacaw_workspace_bytes for the given largest call sizes (keys: SIZE_KEYS)."""
+        z = _Sizes(*[int(sizes.get(k, 0)) for k in SIZE_KEYS])
+        return int(self.lib.tacaw_workspace_bytes(self._ctx, C.byref(z)))
+
+    def set_workspace(self, tensor, **sizes):
+        """tacaw_set_workspace: hand the library a caller-owned CUDA uint8 tensor (kept alive by this object)."""
+        z = _Sizes(*[int(sizes.get(k, 0)) for k in SIZE_KEYS])
+        nbytes = tensor.numel() * tensor.element_size() if tensor is not None else 0
+        rc = self.lib.tacaw_set_workspace(self._ctx, C.c_void_p(tensor.data_ptr()) if tensor is not None else None,
+                                          C.c_size_t(nbytes), C.byref(z))
+        self._check(rc, "tacaw_set_workspace")
+        self._ws = tensor
+        self._ws_sizes = {k: int(sizes.get(k, 0)) for k in SIZE_KEYS}
+
+    def reserve(self, **sizes):
+        """Caller-side convenience: make sure the workspace covers calls of these sizes (grow-only; the library itself
+        never allocates).  Growing allocates a new torch tensor on the current stream and hands it over; work already
+        queued against the old one is ordered before the next call because a context is driven from one stream."""
+        if all(int(sizes.get(k, 0)) <= self._ws_sizes[k] for k in SIZE_KEYS) and self._ws is not None:
+            return
+        new = {k: max(int(sizes.get(k, 0)), self._ws_sizes[k]) for k in SIZE_KEYS}
+        nbytes = self.workspace_bytes(**new)
+        t = self.torch.empty(nbytes + 256, dtype=self.torch.uint8, device=f"cuda:{self.device}")
+        off = (-t.data_ptr()) % 256
+        self.set_workspace(t[off:off + nbytes], **new)
+        self._ws_base = t
+
+    def device_status(self):
+        """tacaw_device_status: synchronises the current stream; raises if a kernel flagged bad input."""
+        self._check(self.lib.tacaw_device_status(self._ctx, self._stream()), "tacaw_device_status")
 
     def close(self):
         if getattr(self, "_ctx", None) is not None and self._ctx.value:
@@ -154,6 +199,7 @@ class Tacaw:
             raise TacawError("build_slices: output tensor has the wrong size")
         sp, keep = self._species(a, b)
         ncl = C.c_int(0)
+        self.reserve(natoms=natoms, nframes=nframes, nslices=nslices)
         rc = self.lib.tacaw_build_slices(self._ctx, self._dev(pos, torch.float64, "pos"),
                                          self._dev(species, torch.int32, "species"), C.c_int(natoms), C.c_int(nframes),
                                          C.byref(sp), C.c_double(dz), C.c_int(nslices), C.c_double(z0),
@@ -163,7 +209,7 @@ class Tacaw:
         return out, (int(ncl.value) if want_clamped else None)
 
     def build_slices_host(self, pos_h: np.ndarray, species_h: np.ndarray, a, b, dz: float, nslices: int,
-                          z0: float, out):
+                          z0: float, out, want_clamped: bool = True):
         """tacaw_build_slices_host: positions [F][Na][3] / species are HOST arrays (H2D inside the call)."""
         torch = self.torch
         pos_h = np.ascontiguousarray(pos_h, dtype=np.float64)
@@ -174,18 +220,21 @@ class Tacaw:
             raise TacawError("build_slices_host: output tensor has the wrong size")
         sp, keep = self._species(a, b)
         ncl = C.c_int(0)
+        self.reserve(natoms=natoms, nframes=nframes, nslices=nslices, host_staging=1)
         rc = self.lib.tacaw_build_slices_host(self._ctx, pos_h.ctypes.data_as(C.c_void_p),
                                               species_h.ctypes.data_as(C.c_void_p), C.c_int(natoms), C.c_int(nframes),
                                               C.byref(sp), C.c_double(dz), C.c_int(nslices), C.c_double(z0),
-                                              self._dev(out, torch.complex64, "trans"), C.byref(ncl), self._stream())
+                                              self._dev(out, torch.complex64, "trans"),
+                                              C.byref(ncl) if want_clamped else None, self._stream())
         self._check(rc, "tacaw_build_slices_host")
-        return out, int(ncl.value)
+        return out, (int(ncl.value) if want_clamped else None)
 
     def make_probes(self, probe_xy: np.ndarray, alpha_rad: float, out=None):
         torch = self.torch
         xy = np.ascontiguousarray(probe_xy, dtype=np.float64).reshape(-1, 2)
         if out is None:
             out = torch.empty((xy.shape[0], self.ny, self.nx), dtype=torch.complex64, device=f"cuda:{self.device}")
+        self.reserve(nprobes=xy.shape[0])
         rc = self.lib.tacaw_make_probes(self._ctx, xy.ctypes.data_as(C.c_void_p), C.c_int(xy.shape[0]),
                                         C.c_double(alpha_rad), self._dev(out, torch.complex64, "waves"), self._stream())
         self._check(rc, "tacaw_make_probes")
@@ -212,10 +261,10 @@ class Tacaw:
         wp = _i32(wave_probe) if wave_probe is not None else None
         if wf.size != nw or (wp is not None and wp.size != nw):
             raise TacawError("wave_frame / wave_probe length mismatch")
-        if probes is not None and wp is not None and wp.size and int(wp.max()) >= probes.shape[0]:
-            raise TacawError("wave_probe out of range")
+        self.reserve(nwaves=nw, nframes=nframes, nsegments=nseg)
         rc = self.lib.tacaw_propagate(self._ctx, self._dev(waves, torch.complex64, "waves"),
                                       self._dev(probes, torch.complex64, "probes") if probes is not None else None,
+                                      C.c_int(int(probes.shape[0]) if probes is not None else 0),
                                       wp.ctypes.data_as(C.c_void_p) if wp is not None else None,
                                       wf.ctypes.data_as(C.c_void_p), C.c_int(nw), ptrs, C.c_int(nframes),
                                       nsl.ctypes.data_as(C.c_void_p), C.c_int(nseg), C.c_double(dz), C.c_int(output_space),
@@ -227,6 +276,7 @@ class Tacaw:
         """tacaw_accumulate: buf (CUDA complex64 [P][T][Q]) updated in place."""
         torch = self.torch
         wp, wf = _i32(wave_probe), _i32(wave_frame)
+        self.reserve(nwaves=qwaves.shape[0])
         rc = self.lib.tacaw_accumulate(self._ctx, self._dev(qwaves, torch.complex64, "qwaves"), C.c_int(qwaves.shape[0]),
                                        wp.ctypes.data_as(C.c_void_p), wf.ctypes.data_as(C.c_void_p),
                                        self._dev(roi_idx, torch.int32, "roi_idx"), C.c_int64(roi_idx.numel()),
@@ -244,6 +294,7 @@ class Tacaw:
         E = np.empty(T, dtype=np.float64)
         args = [C.c_int(P), C.c_int64(Q), C.c_int(T), C.c_double(dt_fs), C.c_int(window), C.c_double(temperature_K),
                 C.c_double(emin), C.c_double(emax)]
+        self.reserve()
         rc = self.lib.tacaw_spectrum(self._ctx, None, *args, None, E.ctypes.data_as(C.c_void_p), C.byref(nE), self._stream())
         self._check(rc, "tacaw_spectrum")
         if out is None:
@@ -255,7 +306,7 @@ class Tacaw:
         return out, E[: nE.value].copy()
 
     def spectrum_welch(self, buf, chunk_len: int, chunk_overlap: int, dt_fs: float, window_table, temperature_K: float,
-                       emin: float = -np.inf, emax: float = np.inf, out=None):
+                       emin: float = -np.inf, emax: float = np.inf, out=None, skip_init: int = 0, stride: int = 1):
         """tacaw_spectrum_welch: returns (I float32 CUDA [P][nE][Q] averaged over the chunks, E float64 numpy [nE], nchunks)."""
         torch = self.torch
         P, Ttot, Q = buf.shape
@@ -264,8 +315,10 @@ class Tacaw:
             raise ValueError("window_table must have chunk_len entries")
         nE, nch = C.c_int(0), C.c_int(0)
         E = np.empty(chunk_len, dtype=np.float64)
-        args = [C.c_int(P), C.c_int64(Q), C.c_int(Ttot), C.c_int(chunk_len), C.c_int(chunk_overlap), C.c_double(dt_fs),
+        args = [C.c_int(P), C.c_int64(Q), C.c_int(Ttot), C.c_int(chunk_len), C.c_int(chunk_overlap), C.c_int(skip_init),
+                C.c_int(stride), C.c_double(dt_fs),
                 w.ctypes.data_as(C.c_void_p), C.c_double(temperature_K), C.c_double(emin), C.c_double(emax)]
+        self.reserve()
         rc = self.lib.tacaw_spectrum_welch(self._ctx, None, *args, None, E.ctypes.data_as(C.c_void_p), C.byref(nE), C.byref(nch),
                                            self._stream())
         self._check(rc, "tacaw_spectrum_welch")
@@ -313,7 +366,7 @@ def make_detector(nx: int, ny: int, lx: float, ly: float, lam: float, kind: str,
 
 
 def make_window(kind: str, n: int, param: float = 0.0) -> np.ndarray:
-    """tacaw_make_window (host): fp64 table of a periodic window ('rect', 'hann', 'tukey', 'blackman_harris', 'kaiser')."""
+    """tacaw_make_window (host): fp64 table of a periodic window ('rect', 'hann', 'tukey', 'blackman_harris', 'kaiser', 'dolph_chebyshev')."""
     lib = load_library()
     w = np.empty(n, dtype=np.float64)
     rc = lib.tacaw_make_window(C.c_int(WINDOWS[kind]), C.c_int(n), C.c_double(param), w.ctypes.data_as(C.c_void_p))

@@ -20,45 +20,57 @@ int cuda_fail(tacaw_ctx* ctx, cudaError_t e, const char* where) {
     return TACAW_E_CUDA;
 }
 
-int ensure(tacaw_ctx* ctx, void** p, size_t* cur, size_t need) {
-    if (*cur >= need) return TACAW_OK;
-    // the old block may still be in use by work queued on a stream: drain before freeing
-    if (*p) {
-        cudaDeviceSynchronize();
-        cudaFree(*p);
-        *p = nullptr;
-        *cur = 0;
-    }
-    size_t sz = need + need / 4 + 256;
-    cudaError_t e = cudaMalloc(p, sz);
-    if (e != cudaSuccess) {
-        (void)cudaGetLastError();
-        return fail(ctx, TACAW_E_NOMEM, "scratch allocation failed");
-    }
-    *cur = sz;
+int region(tacaw_ctx* ctx, int r, size_t need, void** out, const char* who) {
+    if (need == 0) { *out = ctx->d_ws ? ctx->d_ws + ctx->reg_off[r] : nullptr; return TACAW_OK; }
+    if (!ctx->d_ws) return fail(ctx, TACAW_E_NOMEM, std::string(who) + ": no workspace set (tacaw_workspace_bytes / tacaw_set_workspace)");
+    if (ctx->reg_bytes[r] < need)
+        return fail(ctx, TACAW_E_NOMEM, std::string(who) + ": workspace region too small (" + std::to_string(ctx->reg_bytes[r]) + " < " +
+                                            std::to_string(need) + " bytes): size it for this call with tacaw_workspace_bytes");
+    *out = ctx->d_ws + ctx->reg_off[r];
     return TACAW_OK;
 }
 
+// Region sizes for the largest calls a caller announces (tacaw_sizes).  Every region is a multiple of 256 bytes.
+static void region_sizes(const tacaw_ctx* ctx, const tacaw_sizes& z, size_t (&bytes)[tacaw_ctx::R_COUNT]) {
+    auto up = [](size_t v) { return (v + 255) / 256 * 256; };
+    const size_t natoms = (size_t)(z.natoms > 0 ? z.natoms : 0), nframes = (size_t)(z.nframes > 0 ? z.nframes : 0);
+    const size_t nslices = (size_t)(z.nslices > 0 ? z.nslices : 0), nseg = (size_t)(z.nsegments > 0 ? z.nsegments : 1);
+    const size_t nwaves = (size_t)(z.nwaves > 0 ? z.nwaves : 0), nprobes = (size_t)(z.nprobes > 0 ? z.nprobes : 0);
+    const size_t nt = natoms * nframes > 0 ? natoms * nframes : 1, nkeys = nframes * nslices * MAX_SPECIES;
+    // build_slices: clamp counter | keys ux uy sx sy [nt] | counts [nkeys] offsets [nkeys+1]
+    bytes[tacaw_ctx::R_BUILD] = up(256 + sizeof(int) * (5 * nt + 2 * nkeys + 2));
+    bytes[tacaw_ctx::R_STAGE] = z.host_staging ? up(sizeof(double) * 3 * natoms * nframes + sizeof(int32_t) * natoms + 64) : 0;
+    bytes[tacaw_ctx::R_PROBE] = up(sizeof(int) * (size_t)ctx->grid.nx + sizeof(uint32_t) * 2 * nprobes + 64);
+    // propagate: wave_frame | wave_probe | tuples (<= (nwaves + 64) * rpt) | transmission pointers
+    const size_t rpt = (size_t)row_tuple_size(ctx->grid.nx);
+    bytes[tacaw_ctx::R_PROP] = up(sizeof(int) * (2 * nwaves + (nwaves + 64) * rpt) + 16 + sizeof(void*) * nframes * nseg + 64);
+    bytes[tacaw_ctx::R_ACC] = up(sizeof(int) * 2 * nwaves + 64);
+    bytes[tacaw_ctx::R_SPEC] = up(SPEC_TABLE_BYTES);
+}
+
+// Two-half pinned arena: a half is reused only after the copies issued from it have completed (event), never by
+// draining the device.
 int upload(tacaw_ctx* ctx, void* dst, const void* src, size_t bytes, cudaStream_t st) {
     if (bytes == 0) return TACAW_OK;
-    if (!ctx->h_arena) {
-        if (cudaMallocHost((void**)&ctx->h_arena, (size_t)4 << 20) == cudaSuccess) ctx->arena_bytes = (size_t)4 << 20;
-        else (void)cudaGetLastError();
-    }
-    size_t need = (bytes + 63) / 64 * 64;
-    if (need > ctx->arena_bytes) {   // pageable copy: staged by the runtime before it returns
+    const size_t need = (bytes + 63) / 64 * 64;
+    const size_t half = ctx->arena_bytes / 2;
+    if (!ctx->h_arena || need > half) {   // pageable copy: staged by the runtime before it returns
         TACAW_CUDA(ctx, cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, st));
         return TACAW_OK;
     }
-    if (ctx->arena_off + need > ctx->arena_bytes) {
-        // wrap: every copy issued from the arena so far must have completed
-        TACAW_CUDA(ctx, cudaDeviceSynchronize());
-        ctx->arena_off = 0;
+    int h = ctx->arena_off >= half ? 1 : 0;
+    if (ctx->arena_off + need > (size_t)(h + 1) * half) {
+        // leave this half: mark its copies with an event, enter the other half once ITS copies are done
+        TACAW_CUDA(ctx, cudaEventRecord(ctx->ev_arena[h], st));
+        ctx->arena_used[h] = true;
+        h ^= 1;
+        if (ctx->arena_used[h]) TACAW_CUDA(ctx, cudaEventSynchronize(ctx->ev_arena[h]));
+        ctx->arena_off = (size_t)h * half;
     }
-    char* h = ctx->h_arena + ctx->arena_off;
+    char* hp = ctx->h_arena + ctx->arena_off;
     ctx->arena_off += need;
-    memcpy(h, src, bytes);
-    TACAW_CUDA(ctx, cudaMemcpyAsync(dst, h, bytes, cudaMemcpyHostToDevice, st));
+    memcpy(hp, src, bytes);
+    TACAW_CUDA(ctx, cudaMemcpyAsync(dst, hp, bytes, cudaMemcpyHostToDevice, st));
     return TACAW_OK;
 }
 
@@ -76,8 +88,8 @@ static bool supported_n(int n) { return n >= 16 && n <= 2048 && (n & (n - 1)) ==
 
 // twiddle table of the slice-step transforms of length n (layout: fft2.cuh)
 static void make_roots(int n, std::vector<float2>& out) {
-    out.resize(fft2_table_elems(n));
-    fft2_host_table(n, out.data());
+    out.resize(slice_step_table_elems(n));
+    slice_step_host_table(n, out.data());
 }
 
 static int ensure_propagator(tacaw_ctx* ctx, double dz, cudaStream_t st) {
@@ -94,10 +106,11 @@ static int ensure_propagator(tacaw_ctx* ctx, double dz, cudaStream_t st) {
         double ang = -M_PI * ctx->beam.lambda_A * dz * (k / g.ly_A) * (k / g.ly_A);
         py[iy] = make_float2((float)(std::cos(ang) / g.ny), (float)(std::sin(ang) / g.ny));
     }
-    // tables may be in use by queued kernels of a previous dz on another stream: order on `st`
-    TACAW_CUDA(ctx, cudaStreamSynchronize(st));
-    TACAW_CUDA(ctx, cudaMemcpy(ctx->d_px, px.data(), sizeof(float2) * g.nx, cudaMemcpyHostToDevice));
-    TACAW_CUDA(ctx, cudaMemcpy(ctx->d_py, py.data(), sizeof(float2) * g.ny, cudaMemcpyHostToDevice));
+    // stream-ordered: kernels already queued on `st` with the previous dz finish before the copy (a context is driven from
+    // one stream at a time, tacaw.h)
+    int rc = upload(ctx, ctx->d_px, px.data(), sizeof(float2) * g.nx, st);
+    if (rc) return rc;
+    if ((rc = upload(ctx, ctx->d_py, py.data(), sizeof(float2) * g.ny, st))) return rc;
     ctx->dz_cached = dz;
     return TACAW_OK;
 }
@@ -124,11 +137,12 @@ int tacaw_create(tacaw_ctx** out, const tacaw_grid* grid, const tacaw_beam* beam
         (void)cudaGetLastError();
         return TACAW_E_CUDA;
     }
-    if (cudaSetDevice(device) != cudaSuccess) return TACAW_E_CUDA;
     tacaw_ctx* ctx = new tacaw_ctx();
     ctx->grid = *grid;
     ctx->beam = *beam;
     ctx->device = device;
+    DeviceGuard guard(ctx);           // the caller's current device is restored on return
+    if (!guard.ok) { delete ctx; return TACAW_E_CUDA; }
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) == cudaSuccess) {
         ctx->num_sms = prop.multiProcessorCount;
@@ -141,17 +155,26 @@ int tacaw_create(tacaw_ctx** out, const tacaw_grid* grid, const tacaw_beam* beam
     ctx->hmax = 0;
     ctx->hmax_pot = 0;
     ctx->kmaxmax_pot = 0;
+    // per column: the in-band k form an interval |k| <= km (the mask is a disc, monotone in |k|): bisect for km instead
+    // of testing every cell.  Potential extents additionally exclude the Nyquist row and column (reading G4).
     for (int ix = 0; ix < nx; ++ix) {
-        int h = sgn_index(ix, nx);
-        int km = -1, kp = -1;
-        for (int k = 0; k <= ny / 2; ++k) {
-            bool in = beam->bandlimit ? mask_in_band(h, k, *grid) : true;
-            if (in) km = k;
-            if (in && 2 * k < ny && 2 * h != -nx) kp = k;
+        const int h = sgn_index(ix, nx);
+        int km = -1;
+        if (!beam->bandlimit) km = ny / 2;
+        else if (mask_in_band(h, 0, *grid)) {
+            int lo = 0, hi = ny / 2 + 1;              // invariant: in(lo), !in(hi) (k = ny/2 + 1 is outside any 2/3 disc)
+            while (hi - lo > 1) {
+                const int mid = (lo + hi) / 2;
+                if (mid <= ny / 2 && mask_in_band(h, mid, *grid)) lo = mid; else hi = mid;
+            }
+            km = lo;
         }
+        int kp = km;
+        if (2 * kp >= ny) kp = (ny - 1) / 2;          // largest |k| below Nyquist
+        if (2 * h == -nx) kp = -1;
         ctx->kmax[ix] = km;
         ctx->kmax_pot[ix] = kp;
-        int ah = h < 0 ? -h : h;
+        const int ah = h < 0 ? -h : h;
         if (km >= 0 && ah > ctx->hmax) ctx->hmax = ah;
         if (kp >= 0 && ah > ctx->hmax_pot) ctx->hmax_pot = ah;
         if (kp > ctx->kmaxmax_pot) ctx->kmaxmax_pot = kp;
@@ -165,7 +188,12 @@ int tacaw_create(tacaw_ctx** out, const tacaw_grid* grid, const tacaw_beam* beam
               cudaMalloc(&ctx->d_kmax, sizeof(int) * nx) == cudaSuccess &&
               cudaMalloc(&ctx->d_kmax_pot, sizeof(int) * nx) == cudaSuccess &&
               cudaMalloc(&ctx->d_px, sizeof(float2) * nx) == cudaSuccess &&
-              cudaMalloc(&ctx->d_py, sizeof(float2) * ny) == cudaSuccess;
+              cudaMalloc(&ctx->d_py, sizeof(float2) * ny) == cudaSuccess &&
+              cudaMalloc(&ctx->d_flags, 4 * sizeof(int)) == cudaSuccess &&
+              cudaMemset(ctx->d_flags, 0, 4 * sizeof(int)) == cudaSuccess;
+    if (cudaMallocHost((void**)&ctx->h_arena, (size_t)8 << 20) == cudaSuccess) ctx->arena_bytes = (size_t)8 << 20;
+    else { (void)cudaGetLastError(); ctx->h_arena = nullptr; }
+    for (int i = 0; i < 2; ++i) ok = ok && cudaEventCreateWithFlags(&ctx->ev_arena[i], cudaEventDisableTiming) == cudaSuccess;
     ok = ok && cudaMemcpy(ctx->d_roots_x, rx.data(), sizeof(float2) * rx.size(), cudaMemcpyHostToDevice) == cudaSuccess &&
          cudaMemcpy(ctx->d_roots_y, ry.data(), sizeof(float2) * ry.size(), cudaMemcpyHostToDevice) == cudaSuccess &&
          cudaMemcpy(ctx->d_kmax, ctx->kmax.data(), sizeof(int) * nx, cudaMemcpyHostToDevice) == cudaSuccess &&
@@ -185,25 +213,67 @@ int tacaw_create(tacaw_ctx** out, const tacaw_grid* grid, const tacaw_beam* beam
 
 int tacaw_destroy(tacaw_ctx* ctx) {
     if (!ctx) return TACAW_E_ARG;
-    cudaDeviceSynchronize();
-    cudaFree(ctx->d_roots_x); cudaFree(ctx->d_roots_y); cudaFree(ctx->d_kmax); cudaFree(ctx->d_kmax_pot);
-    cudaFree(ctx->d_px); cudaFree(ctx->d_py); cudaFree(ctx->d_meta); cudaFree(ctx->d_sort); cudaFree(ctx->d_stage);
-    cudaFree(ctx->d_spec_tab);
-    if (ctx->h_arena) cudaFreeHost(ctx->h_arena);
-    for (int i = 0; i < tacaw_ctx::MAX_AUX; ++i) {
-        if (ctx->aux[i]) cudaStreamDestroy(ctx->aux[i]);
-        if (ctx->ev_join[i]) cudaEventDestroy(ctx->ev_join[i]);
+    {
+        DeviceGuard guard(ctx);
+        cudaDeviceSynchronize();
+        cudaFree(ctx->d_roots_x); cudaFree(ctx->d_roots_y); cudaFree(ctx->d_kmax); cudaFree(ctx->d_kmax_pot);
+        cudaFree(ctx->d_px); cudaFree(ctx->d_py); cudaFree(ctx->d_flags);      // the workspace is the caller's
+        if (ctx->h_arena) cudaFreeHost(ctx->h_arena);
+        for (int i = 0; i < 2; ++i)
+            if (ctx->ev_arena[i]) cudaEventDestroy(ctx->ev_arena[i]);
+        for (int i = 0; i < tacaw_ctx::MAX_AUX; ++i) {
+            if (ctx->aux[i]) cudaStreamDestroy(ctx->aux[i]);
+            if (ctx->ev_join[i]) cudaEventDestroy(ctx->ev_join[i]);
+        }
+        if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+        (void)cudaGetLastError();
     }
-    if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
-    (void)cudaGetLastError();
     delete ctx;
+    return TACAW_OK;
+}
+
+size_t tacaw_workspace_bytes(const tacaw_ctx* ctx, const tacaw_sizes* sizes) {
+    if (!ctx || !sizes) return 0;
+    size_t b[tacaw_ctx::R_COUNT];
+    region_sizes(ctx, *sizes, b);
+    size_t tot = 0;
+    for (int r = 0; r < tacaw_ctx::R_COUNT; ++r) tot += b[r];
+    return tot;
+}
+
+int tacaw_set_workspace(tacaw_ctx* ctx, void* d_workspace, size_t bytes, const tacaw_sizes* sizes) {
+    TACAW_ENTER(ctx);
+    if (!sizes || (!d_workspace && bytes > 0)) return fail(ctx, TACAW_E_ARG, "tacaw_set_workspace: bad argument");
+    if (((uintptr_t)d_workspace & 255) != 0) return fail(ctx, TACAW_E_ARG, "tacaw_set_workspace: the workspace must be 256-byte aligned");
+    size_t b[tacaw_ctx::R_COUNT];
+    region_sizes(ctx, *sizes, b);
+    size_t tot = 0;
+    for (int r = 0; r < tacaw_ctx::R_COUNT; ++r) tot += b[r];
+    if (bytes < tot) return fail(ctx, TACAW_E_NOMEM, "tacaw_set_workspace: " + std::to_string(bytes) + " bytes given, " + std::to_string(tot) + " needed for these sizes");
+    ctx->d_ws = (char*)d_workspace;
+    ctx->ws_bytes = bytes;
+    size_t off = 0;
+    for (int r = 0; r < tacaw_ctx::R_COUNT; ++r) { ctx->reg_off[r] = off; ctx->reg_bytes[r] = b[r]; off += b[r]; }
+    ctx->maps.clear();
+    return TACAW_OK;
+}
+
+int tacaw_device_status(tacaw_ctx* ctx, void* stream) {
+    TACAW_ENTER(ctx);
+    int h[4] = {0, 0, 0, 0};
+    TACAW_CUDA(ctx, cudaMemcpyAsync(h, ctx->d_flags, sizeof(h), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+    TACAW_CUDA(ctx, cudaStreamSynchronize((cudaStream_t)stream));
+    if (h[0] > 0) {
+        TACAW_CUDA(ctx, cudaMemsetAsync(ctx->d_flags, 0, sizeof(h), (cudaStream_t)stream));
+        return fail(ctx, TACAW_E_ARG, "tacaw_build_slices: " + std::to_string(h[0]) + " species id(s) out of range since the last status check");
+    }
     return TACAW_OK;
 }
 
 int tacaw_build_slices(tacaw_ctx* ctx, const double* d_pos_A, const int32_t* d_species, int natoms, int nframes,
                        const tacaw_species* species, double dz, int nslices, double z0, void* d_trans, int* n_clamped,
                        void* stream) {
-    if (!ctx) return TACAW_E_ARG;
+    TACAW_ENTER(ctx);
     if (nframes == 0) { if (n_clamped) *n_clamped = 0; return TACAW_OK; }
     if (natoms < 0 || nframes < 0 || nslices <= 0 || !(dz > 0) || !d_trans || !species || species->nspecies <= 0 || !species->a ||
         !species->b || (natoms > 0 && (!d_pos_A || !d_species)))
@@ -212,16 +282,14 @@ int tacaw_build_slices(tacaw_ctx* ctx, const double* d_pos_A, const int32_t* d_s
     const int ns = species->nspecies;
     const int nx = ctx->grid.nx, ny = ctx->grid.ny;
     if (ns > MAX_SPECIES) return fail(ctx, TACAW_E_UNSUPPORTED, "tacaw_build_slices: at most 8 species");
-    int rc = ensure(ctx, &ctx->d_meta, &ctx->meta_bytes, 4096);
-    if (rc) return rc;
     AbTable ab{};
     for (int s = 0; s < ns; ++s)
         for (int i = 0; i < 4; ++i) {
             ab.a[s][i] = (float)species->a[4 * s + i];
             ab.b[s][i] = (float)species->b[4 * s + i];
         }
-    int* d_ncl = (int*)ctx->d_meta;   // [0] clamped atoms, [1] bad species ids
-    rc = launch_potential(ctx, d_pos_A, d_species, natoms, nframes, ns, ab, dz, nslices, z0, (float2*)d_trans, d_ncl, st);
+    int* d_ncl = nullptr;             // clamped atoms of this call (first word of the build region)
+    int rc = launch_potential(ctx, d_pos_A, d_species, natoms, nframes, ns, ab, dz, nslices, z0, (float2*)d_trans, &d_ncl, st);
     if (rc) return rc;
     // V(q) -> v(r) -> t = exp(i sigma v):  IFFT_y over the in-band columns, then IFFT_x + exp per row
     ColArgs ca{};
@@ -234,12 +302,13 @@ int tacaw_build_slices(tacaw_ctx* ctx, const double* d_pos_A, const int32_t* d_s
     ra.scale = (float)(ctx->beam.sigma_rad_per_VA / (ctx->grid.lx_A * ctx->grid.ly_A));
     rc = launch_row(ctx, ROW_TRANS, ra, st);
     if (rc) return rc;
-    int h_ncl[2] = {0, 0};
     if (n_clamped) {
-        TACAW_CUDA(ctx, cudaMemcpyAsync(h_ncl, d_ncl, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
+        // the one synchronising path: also reports (and clears) the sticky species-id flag
+        int h_ncl = 0;
+        TACAW_CUDA(ctx, cudaMemcpyAsync(&h_ncl, d_ncl, sizeof(int), cudaMemcpyDeviceToHost, st));
         TACAW_CUDA(ctx, cudaStreamSynchronize(st));
-        *n_clamped = h_ncl[0];
-        if (h_ncl[1] > 0) return fail(ctx, TACAW_E_ARG, "tacaw_build_slices: species id out of range");
+        *n_clamped = h_ncl;
+        return tacaw_device_status(ctx, stream);
     }
     return TACAW_OK;
 }
@@ -247,27 +316,30 @@ int tacaw_build_slices(tacaw_ctx* ctx, const double* d_pos_A, const int32_t* d_s
 int tacaw_build_slices_host(tacaw_ctx* ctx, const double* h_pos_A, const int32_t* h_species, int natoms, int nframes,
                             const tacaw_species* species, double dz, int nslices, double z0, void* d_trans,
                             int* n_clamped, void* stream) {
-    if (!ctx) return TACAW_E_ARG;
-    if (natoms < 0 || nframes < 0 || (natoms > 0 && nframes > 0 && (!h_pos_A || !h_species))) return fail(ctx, TACAW_E_ARG, "bad argument");
+    TACAW_ENTER(ctx);
+    if (natoms < 0 || nframes < 0 || !species || (natoms > 0 && nframes > 0 && (!h_pos_A || !h_species))) return fail(ctx, TACAW_E_ARG, "bad argument");
+    // species ids are on the host here: validate them before anything is queued
+    for (int j = 0; j < natoms; ++j)
+        if (h_species[j] < 0 || h_species[j] >= species->nspecies) return fail(ctx, TACAW_E_ARG, "tacaw_build_slices_host: species id out of range");
     cudaStream_t st = (cudaStream_t)stream;
     size_t nb_pos = sizeof(double) * 3 * (size_t)natoms * (size_t)nframes, nb_sp = sizeof(int32_t) * (size_t)natoms;
-    int rc = ensure(ctx, &ctx->d_stage, &ctx->stage_bytes, nb_pos + nb_sp + 64);
+    void* stage = nullptr;
+    int rc = region(ctx, tacaw_ctx::R_STAGE, nb_pos + nb_sp + 64, &stage, "tacaw_build_slices_host");
     if (rc) return rc;
-    double* d_pos = (double*)ctx->d_stage;
-    int32_t* d_sp = (int32_t*)((char*)ctx->d_stage + nb_pos);
+    double* d_pos = (double*)stage;
+    int32_t* d_sp = (int32_t*)((char*)stage + nb_pos);
     if (natoms > 0 && nframes > 0) {
         TACAW_CUDA(ctx, cudaMemcpyAsync(d_pos, h_pos_A, nb_pos, cudaMemcpyHostToDevice, st));
         TACAW_CUDA(ctx, cudaMemcpyAsync(d_sp, h_species, nb_sp, cudaMemcpyHostToDevice, st));
     }
-    int dummy = 0;
-    rc = tacaw_build_slices(ctx, d_pos, d_sp, natoms, nframes, species, dz, nslices, z0, d_trans, n_clamped ? n_clamped : &dummy,
-                            stream);
-    return rc;
+    // n_clamped == NULL: nothing to read back, the call stays asynchronous (pinned sources; pageable ones are staged by
+    // the runtime before cudaMemcpyAsync returns)
+    return tacaw_build_slices(ctx, d_pos, d_sp, natoms, nframes, species, dz, nslices, z0, d_trans, n_clamped, stream);
 }
 
 int tacaw_make_probes(tacaw_ctx* ctx, const double* probe_xy_A, int nprobes, double alpha_rad, void* d_waves,
                       void* stream) {
-    if (!ctx) return TACAW_E_ARG;
+    TACAW_ENTER(ctx);
     if (nprobes < 0 || (nprobes > 0 && (!probe_xy_A || !d_waves)) || alpha_rad < 0)
         return fail(ctx, TACAW_E_ARG, "tacaw_make_probes: bad argument");
     if (nprobes == 0) return TACAW_OK;
@@ -305,9 +377,10 @@ int tacaw_make_probes(tacaw_ctx* ctx, const double* probe_xy_A, int nprobes, dou
         uxy[2 * p + 1] = (uint32_t)(unsigned long long)std::llrint(fy * 4294967296.0);
     }
     size_t need = sizeof(int) * nx + sizeof(uint32_t) * uxy.size() + 64;
-    int rc = ensure(ctx, &ctx->d_meta, &ctx->meta_bytes, need > 4096 ? need : 4096);
+    void* reg = nullptr;
+    int rc = region(ctx, tacaw_ctx::R_PROBE, need, &reg, "tacaw_make_probes");
     if (rc) return rc;
-    int* d_kap = (int*)ctx->d_meta;
+    int* d_kap = (int*)reg;
     uint32_t* d_uxy = (uint32_t*)(d_kap + nx);
     if ((rc = upload(ctx, d_kap, kap.data(), sizeof(int) * nx, st))) return rc;
     if ((rc = upload(ctx, d_uxy, uxy.data(), sizeof(uint32_t) * uxy.size(), st))) return rc;
@@ -324,17 +397,17 @@ int tacaw_make_probes(tacaw_ctx* ctx, const double* probe_xy_A, int nprobes, dou
     ra.waves = (float2*)d_waves; ra.nwaves = nprobes; ra.ny = ny; ra.hmax = hap; ra.roots = ctx->d_roots_x;
     rc = launch_row(ctx, ROW_LAST, ra, st);
     if (rc) return rc;
-    // d_meta is reused by later calls: make sure the fill kernel has consumed it
-    TACAW_CUDA(ctx, cudaStreamSynchronize(st));
+    // the probe region is private to this entry point and reuse is stream-ordered: no synchronisation
     return TACAW_OK;
 }
 
-int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, const int32_t* wave_probe,
+int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, int nprobes, const int32_t* wave_probe,
                     const int32_t* wave_frame, int nwaves, const void* const* d_trans, int nframes,
                     const int32_t* nslices_per_segment, int nsegments, double dz, int output_space, void* stream) {
-    if (!ctx) return TACAW_E_ARG;
+    TACAW_ENTER(ctx);
     if (nwaves < 0 || nframes <= 0 || nsegments <= 0 || !(dz > 0) || !d_trans || !nslices_per_segment ||
-        (nwaves > 0 && (!d_waves || !wave_frame)) || (d_probes && !wave_probe) || (output_space != 0 && output_space != 1))
+        (nwaves > 0 && (!d_waves || !wave_frame)) || (d_probes && (!wave_probe || nprobes <= 0)) ||
+        (output_space != 0 && output_space != 1))
         return fail(ctx, TACAW_E_ARG, "tacaw_propagate: bad argument");
     if (nwaves == 0) return TACAW_OK;
     int total = 0;
@@ -345,7 +418,7 @@ int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, const i
     if (total == 0) return fail(ctx, TACAW_E_ARG, "tacaw_propagate: no slices");
     for (int w = 0; w < nwaves; ++w) {
         if (wave_frame[w] < 0 || wave_frame[w] >= nframes) return fail(ctx, TACAW_E_ARG, "wave_frame out of range");
-        if (d_probes && wave_probe[w] < 0) return fail(ctx, TACAW_E_ARG, "wave_probe out of range");
+        if (d_probes && (wave_probe[w] < 0 || wave_probe[w] >= nprobes)) return fail(ctx, TACAW_E_ARG, "wave_probe out of range");
     }
     for (int i = 0; i < nframes * nsegments; ++i)
         if (!d_trans[i] && nslices_per_segment[i % nsegments] > 0) return fail(ctx, TACAW_E_ARG, "null transmission pointer");
@@ -361,12 +434,13 @@ int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, const i
     size_t off_t = 2 * nb_i;
     size_t off_p = ((off_t + nb_t + 15) / 16) * 16;
     size_t need = off_p + sizeof(void*) * (size_t)nframes * nsegments + 64;
-    rc = ensure(ctx, &ctx->d_meta, &ctx->meta_bytes, need > 4096 ? need : 4096);
+    void* meta = nullptr;
+    rc = region(ctx, tacaw_ctx::R_PROP, need, &meta, "tacaw_propagate");
     if (rc) return rc;
-    int* d_wf = (int*)ctx->d_meta;
+    int* d_wf = (int*)meta;
     int* d_wp = d_wf + nwaves;
-    int* d_tup = (int*)((char*)ctx->d_meta + off_t);
-    const float2** d_tp = (const float2**)((char*)ctx->d_meta + off_p);
+    int* d_tup = (int*)((char*)meta + off_t);
+    const float2** d_tp = (const float2**)((char*)meta + off_p);
     if ((rc = upload(ctx, d_wf, wave_frame, nb_i, st))) return rc;
     if (d_probes && (rc = upload(ctx, d_wp, wave_probe, nb_i, st))) return rc;
     if ((rc = upload(ctx, (void*)d_tp, d_trans, sizeof(void*) * (size_t)nframes * nsegments, st))) return rc;
@@ -377,7 +451,7 @@ int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, const i
     // L2/5 (25 MB: 48 waves at 256^2, 12 at 512^2, 3 at 1024^2), swept on B200: 512^2 reaches 0.556 of the roofline with
     // 12 waves per group, 0.54 with 15 (L2/4), 0.53 with 11
     size_t budget = ctx->l2_bytes ? ctx->l2_bytes / 5 : (size_t)25 << 20;
-    int gmin = 3;    // 2048^2: a launch over fewer waves is all fill and drain (measured: 1 wave 0.30, 3 waves 0.32 of the roofline)
+    int gmin = 3;
     if (const char* e = getenv("TACAW_L2_GROUP_MB")) {
         double mb = atof(e);
         if (mb > 0) {
@@ -387,13 +461,18 @@ int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, const i
     }
     int gmax = (int)(budget / (npix * sizeof(float2)));
     if (gmax >= 2 * rpt) gmax -= gmax % rpt;      // whole row tuples: a short tuple repeats its last wave (wasted work)
-    if (gmax < gmin) gmax = gmin;
+    // A wave larger than the budget (2048^2: 33.6 MB, 22.4 MB in band): what stays L2-resident is the TOTAL in flight, and
+    // beyond ~90 MB of in-band waves plus the streaming t_n slice (33.6 MB) the 126 MB L2 thrashes.  Swept on B200 (streams x
+    // waves per group, fraction of the roofline): 1x3 0.326, 2x2 0.346, 2x3 0.333, 3x2 0.326, 3x3 0.331, any x4 0.27-0.28.
+    const bool huge = gmax < 2;
+    if (gmax < gmin) gmax = huge ? 2 : gmin;
     const int ngroups = (nwaves + gmax - 1) / gmax;
-    static const int max_streams = [] {
+    static const int env_streams = [] {
         const char* e = getenv("TACAW_STREAMS");
-        int v = e ? atoi(e) : 3;
-        return v < 1 ? 1 : (v > 1 + tacaw_ctx::MAX_AUX ? 1 + tacaw_ctx::MAX_AUX : v);
+        int v = e ? atoi(e) : 0;
+        return v < 0 ? 0 : (v > 1 + tacaw_ctx::MAX_AUX ? 1 + tacaw_ctx::MAX_AUX : v);
     }();
+    const int max_streams = env_streams ? env_streams : (huge ? 2 : 3);
     const int nstreams = ngroups < max_streams ? ngroups : max_streams;
     const bool fork = nstreams >= 2;
     cudaStream_t user_st = st;
@@ -449,6 +528,7 @@ int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, const i
                 bool lastq = (step == total - 1) && output_space == 1;
                 ColArgs ca{};
                 ca.waves = ra.waves; ca.nwaves = nw; ca.nx = g.nx; ca.hmax = ctx->hmax; ca.roots = ctx->d_roots_y;
+                ca.stack = (float2*)d_waves; ca.stack_waves = nwaves; ca.wave0 = w0;      // one tensor map for the whole call
                 ca.px = ctx->d_px; ca.py = ctx->d_py; ca.kmax = ctx->d_kmax;
                 ca.pscale = lastq ? (float)((double)g.nx * (double)g.ny) : 1.f;
                 ca.kmaxmax = ctx->kmaxmax;
@@ -475,34 +555,81 @@ int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, const i
     return TACAW_OK;
 }
 
+// O8 by row spans: for a fixed k every predicate is monotone in |h| (disc, annulus) or in h (rect), so the kept h of a row
+// are one or two intervals whose ends are found by bisection on the fp64 predicate value; the cells are then emitted in
+// ascending h.  (The oracle tests every cell; the two enumerators share the definition of theta^2 only.)
+namespace {
+struct RoiPred {
+    const tacaw_grid* g;
+    double lambda;
+    bool square;
+    double theta2(int h, int k) const {
+        if (square) {
+            const double sc = lambda / g->lx_A;
+            return sc * sc * (double)((long long)h * h + (long long)k * k);
+        }
+        return lambda * lambda * ((h / g->lx_A) * (h / g->lx_A) + (k / g->ly_A) * (k / g->ly_A));
+    }
+};
+// largest a in [0, amax] with theta2(a, k) <= lim2, or -1
+int last_le(const RoiPred& p, int k, int amax, double lim2) {
+    if (!(p.theta2(0, k) <= lim2)) return -1;
+    int lo = 0, hi = amax + 1;
+    while (hi - lo > 1) {
+        const int mid = lo + (hi - lo) / 2;
+        if (p.theta2(mid, k) <= lim2) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+// smallest a in [0, amax] with theta2(a, k) >= lim2, or amax + 1
+int first_ge(const RoiPred& p, int k, int amax, double lim2) {
+    if (p.theta2(0, k) >= lim2) return 0;
+    int lo = 0, hi = amax + 1;                       // theta2(lo) < lim2; hi: first candidate not yet excluded
+    while (hi - lo > 1) {
+        const int mid = lo + (hi - lo) / 2;
+        if (p.theta2(mid, k) >= lim2) hi = mid; else lo = mid;
+    }
+    return hi;
+}
+}  // namespace
+
 int tacaw_make_roi(const tacaw_grid* g, double lambda, int mode, const double* params, int32_t* idx_out, int64_t* count) {
     if (!g || !count || g->nx <= 0 || g->ny <= 0 || (mode != TACAW_ROI_FULL && !params)) return TACAW_E_ARG;
     if (mode < 0 || mode > 3) return TACAW_E_ARG;
-    const bool square = (g->nx == g->ny && g->lx_A == g->ly_A);
+    const RoiPred pred{g, lambda, g->nx == g->ny && g->lx_A == g->ly_A};
+    const int hlo = -g->nx / 2, hhi = g->nx - g->nx / 2 - 1;        // signed h range of the grid
+    const int amax = g->nx / 2;                                     // largest |h| (the negative end)
     int64_t c = 0;
-    for (int k = -g->ny / 2; k < g->ny - g->ny / 2; ++k)
-        for (int h = -g->nx / 2; h < g->nx - g->nx / 2; ++h) {
-            bool keep = true;
-            if (mode == TACAW_ROI_DISC || mode == TACAW_ROI_ANNULUS) {
-                double t2;
-                if (square) {
-                    double s = lambda / g->lx_A;
-                    t2 = s * s * (double)((long long)h * h + (long long)k * k);
-                } else {
-                    t2 = lambda * lambda * ((h / g->lx_A) * (h / g->lx_A) + (k / g->ly_A) * (k / g->ly_A));
-                }
-                double to = (mode == TACAW_ROI_DISC) ? params[0] : params[1];
-                keep = t2 <= to * to;
-                if (mode == TACAW_ROI_ANNULUS) keep = keep && t2 >= params[0] * params[0];
-            } else if (mode == TACAW_ROI_RECT) {
-                double tx = lambda * h / g->lx_A, ty = lambda * k / g->ly_A;
-                keep = tx >= params[0] && tx <= params[1] && ty >= params[2] && ty <= params[3];
-            }
-            if (keep) {
-                if (idx_out) idx_out[c] = (int32_t)(((k + g->ny) % g->ny) * g->nx + (h + g->nx) % g->nx);
-                ++c;
-            }
+    auto emit = [&](int k, int h0, int h1) {                        // cells h0..h1 of row k, clipped to the grid
+        if (h0 < hlo) h0 = hlo;
+        if (h1 > hhi) h1 = hhi;
+        for (int h = h0; h <= h1; ++h, ++c)
+            if (idx_out) idx_out[c] = (int32_t)(((k + g->ny) % g->ny) * g->nx + (h + g->nx) % g->nx);
+    };
+    for (int k = -g->ny / 2; k < g->ny - g->ny / 2; ++k) {
+        if (mode == TACAW_ROI_FULL) {
+            emit(k, hlo, hhi);
+        } else if (mode == TACAW_ROI_DISC || mode == TACAW_ROI_ANNULUS) {
+            const double to = (mode == TACAW_ROI_DISC) ? params[0] : params[1];
+            const int aout = last_le(pred, k, amax, to * to);
+            if (aout < 0) continue;
+            int ain = 0;
+            if (mode == TACAW_ROI_ANNULUS) ain = first_ge(pred, k, amax, params[0] * params[0]);
+            if (ain > aout) continue;
+            if (ain == 0) emit(k, -aout, aout);
+            else { emit(k, -aout, -ain); emit(k, ain, aout); }
+        } else {
+            const double ty = lambda * k / g->ly_A;
+            if (!(ty >= params[2] && ty <= params[3])) continue;
+            // lambda*h/lx is increasing in h: first h with tx >= txmin, last h with tx <= txmax
+            int lo = hlo - 1, hi = hhi + 1;
+            while (hi - lo > 1) { const int mid = lo + (hi - lo) / 2; if (lambda * mid / g->lx_A >= params[0]) hi = mid; else lo = mid; }
+            const int h0 = hi;
+            lo = hlo - 1; hi = hhi + 1;
+            while (hi - lo > 1) { const int mid = lo + (hi - lo) / 2; if (lambda * mid / g->lx_A <= params[1]) lo = mid; else hi = mid; }
+            emit(k, h0, lo);
         }
+    }
     *count = c;
     return TACAW_OK;
 }
@@ -510,7 +637,7 @@ int tacaw_make_roi(const tacaw_grid* g, double lambda, int mode, const double* p
 int tacaw_accumulate(tacaw_ctx* ctx, const void* d_qwaves, int nwaves, const int32_t* wave_probe,
                      const int32_t* wave_frame, const int32_t* d_roi_idx, int64_t nroi, void* d_buf, int nprobes,
                      int nframes, void* stream) {
-    if (!ctx) return TACAW_E_ARG;
+    TACAW_ENTER(ctx);
     if (nwaves < 0 || nroi < 0 || nprobes <= 0 || nframes <= 0 ||
         (nwaves > 0 && nroi > 0 && (!d_qwaves || !wave_probe || !wave_frame || !d_roi_idx || !d_buf)))
         return fail(ctx, TACAW_E_ARG, "tacaw_accumulate: bad argument");
@@ -519,12 +646,12 @@ int tacaw_accumulate(tacaw_ctx* ctx, const void* d_qwaves, int nwaves, const int
         if (wave_probe[w] < 0 || wave_probe[w] >= nprobes || wave_frame[w] < 0 || wave_frame[w] >= nframes)
             return fail(ctx, TACAW_E_ARG, "tacaw_accumulate: probe/frame index out of range");
     cudaStream_t st = (cudaStream_t)stream;
-    // index arrays go to the staging region (stream-ordered after any earlier user of it)
+    // index arrays go to this entry point's own region (reuse is stream-ordered)
     size_t nb_i = sizeof(int) * (size_t)nwaves;
-    size_t need = 4 * nb_i + 4096;
-    int rc = ensure(ctx, &ctx->d_stage, &ctx->stage_bytes, need);
+    void* reg = nullptr;
+    int rc = region(ctx, tacaw_ctx::R_ACC, 2 * nb_i, &reg, "tacaw_accumulate");
     if (rc) return rc;
-    int* d_wp = (int*)ctx->d_stage;
+    int* d_wp = (int*)reg;
     int* d_wf = d_wp + nwaves;
     if ((rc = upload(ctx, d_wp, wave_probe, nb_i, st))) return rc;
     if ((rc = upload(ctx, d_wf, wave_frame, nb_i, st))) return rc;
@@ -534,9 +661,10 @@ int tacaw_accumulate(tacaw_ctx* ctx, const void* d_qwaves, int nwaves, const int
 
 // Shared core of tacaw_spectrum / tacaw_spectrum_welch: chunks of L frames starting every `step` frames of a
 // [nprobes][nframes_total][nroi] buffer, window table w[L] (fp64, host), I = (1/nchunks) sum_i I_i.
-static int spectrum_core(tacaw_ctx* ctx, const void* d_buf, int nprobes, int64_t nroi, int nframes_total, int L, int step,
-                         int nchunks, double dt_fs, const double* w, double temperature_K, double emin, double emax, float* d_I,
-                         double* E_out, int* nE_out, cudaStream_t st, const char* who) {
+// chunk n starts at frame first + n*step and holds frames first + n*step + f*stride, f = 0..L-1; time step dt_fs (of a chunk).
+static int spectrum_core(tacaw_ctx* ctx, const void* d_buf, int nprobes, int64_t nroi, int nframes_total, int L, int first, int step,
+                         int stride, int nchunks, double dt_fs, const double* w, double temperature_K, double emin, double emax,
+                         float* d_I, double* E_out, int* nE_out, cudaStream_t st, const char* who) {
     if (L < 8 || L > 2048 || (L & (L - 1))) return fail(ctx, TACAW_E_UNSUPPORTED, std::string(who) + ": the transform length must be a power of two in [8, 2048]");
     const double h_mev_fs = 4135.667696, kb_mev = 8.617333262e-2;
     // ascending axis k' = -L/2 .. L/2-1; keep [emin, emax] with 1e-9 meV slack (reading G11)
@@ -576,16 +704,15 @@ static int spectrum_core(tacaw_ctx* ctx, const void* d_buf, int nprobes, int64_t
         double B = (x == 0.0) ? 1.0 : x / (-std::expm1(-x));
         tab[2 * NR + (size_t)L + i] = (float)(B / ((double)L * sw2 * (double)nchunks));
     }
-    int rc = ensure(ctx, (void**)&ctx->d_spec_tab, &ctx->spec_tab_bytes, sizeof(float) * tab.size());
+    void* reg = nullptr;
+    int rc = region(ctx, tacaw_ctx::R_SPEC, sizeof(float) * tab.size(), &reg, who);
     if (rc) return rc;
-    if ((rc = upload(ctx, ctx->d_spec_tab, tab.data(), sizeof(float) * tab.size(), st))) return rc;
-    for (int c = 0; c < nchunks; ++c) {
-        rc = launch_spectrum(ctx, (const float2*)d_buf + (size_t)c * step * (size_t)nroi, nprobes, nroi, L,
-                             (size_t)nframes_total * (size_t)nroi, c > 0, (const float2*)ctx->d_spec_tab,
-                             ctx->d_spec_tab + 2 * NR, ctx->d_spec_tab + 2 * NR + (size_t)L, e_lo, nE, d_I, st);
-        if (rc) return rc;
-    }
-    return TACAW_OK;
+    float* d_spec_tab = (float*)reg;
+    if ((rc = upload(ctx, d_spec_tab, tab.data(), sizeof(float) * tab.size(), st))) return rc;
+    // one launch for all chunks: the kernel sums |Phi_n|^2 over the chunks in registers and writes I once
+    return launch_spectrum(ctx, (const float2*)d_buf + (size_t)first * (size_t)nroi, nprobes, nroi, L,
+                           (size_t)nframes_total * (size_t)nroi, (size_t)stride * (size_t)nroi, nchunks, (size_t)step * (size_t)nroi,
+                           (const float2*)d_spec_tab, d_spec_tab + 2 * NR, d_spec_tab + 2 * NR + (size_t)L, e_lo, nE, d_I, st);
 }
 
 // modified Bessel function I0 (power series; converges for every beta used as a Kaiser parameter)
@@ -600,8 +727,41 @@ static double bessel_i0(double x) {
     return sum;
 }
 
+// Dolph-Chebyshev: periodic form of the M = n + 1 point window whose transform is T_{M-1}(x0 cos(theta/2)):
+// cosine series over the M samples of that transform, centred on the window's midpoint, angles reduced in integer
+// arithmetic before cos(), normalised to its maximum.
+static int dolph_chebyshev(int n, double att_db, double* w_out) {
+    if (!(att_db > 0.0)) return TACAW_E_ARG;
+    const int M = n + 1, m = M - 1;
+    const double x0 = std::cosh(std::acosh(std::pow(10.0, att_db / 20.0)) / (double)m);
+    std::vector<double> Wk(M);
+    for (int k = 0; k < M; ++k) {
+        const double x = x0 * std::cos(M_PI * (double)k / (double)M);
+        double t;
+        if (x > 1.0) t = std::cosh((double)m * std::acosh(x));
+        else if (x < -1.0) t = ((m & 1) ? -1.0 : 1.0) * std::cosh((double)m * std::acosh(-x));
+        else t = std::cos((double)m * std::acos(x));
+        Wk[k] = t;
+    }
+    std::vector<double> w(M);
+    double wmax = 0.0;
+    for (int j = 0; j < M; ++j) {
+        double acc = Wk[0];
+        for (int k = 1; k < M; ++k) {
+            // reduce the angle 2 pi k d / M through the integer 2 k j - k m (mod 2M) before calling cos
+            const long long num = ((2LL * k * j - (long long)k * m) % (2LL * M) + 2LL * M) % (2LL * M);
+            acc += Wk[k] * std::cos(M_PI * (double)num / (double)M);
+        }
+        w[j] = acc;
+        if (acc > wmax) wmax = acc;
+    }
+    for (int f = 0; f < n; ++f) w_out[f] = w[f] / wmax;
+    return TACAW_OK;
+}
+
 int tacaw_make_window(int kind, int n, double param, double* w_out) {
     if (n <= 0 || !w_out) return TACAW_E_ARG;
+    if (kind == TACAW_WINDOW_DOLPH_CHEBYSHEV) return dolph_chebyshev(n, param, w_out);
     for (int f = 0; f < n; ++f) {
         const double x = (double)f / (double)n;          // periodic form: sample f of a window of period n
         double v = 1.0;
@@ -635,31 +795,36 @@ int tacaw_make_window(int kind, int n, double param, double* w_out) {
 
 int tacaw_spectrum(tacaw_ctx* ctx, const void* d_buf, int nprobes, int64_t nroi, int nframes, double dt_fs, int window,
                    double temperature_K, double emin, double emax, float* d_I, double* E_out, int* nE_out, void* stream) {
-    if (!ctx) return TACAW_E_ARG;
+    TACAW_ENTER(ctx);
     if (nprobes < 0 || nroi < 0 || nframes <= 0 || !(dt_fs > 0) || !(temperature_K > 0) || !nE_out ||
         (window != TACAW_WINDOW_RECT && window != TACAW_WINDOW_HANN))
         return fail(ctx, TACAW_E_ARG, "tacaw_spectrum: bad argument");
     if (nframes < 8 || nframes > 2048 || (nframes & (nframes - 1))) return fail(ctx, TACAW_E_UNSUPPORTED, "nframes must be a power of two in [8, 2048]");
     std::vector<double> w(nframes);
     tacaw_make_window(window, nframes, 0.0, w.data());
-    return spectrum_core(ctx, d_buf, nprobes, nroi, nframes, nframes, nframes, 1, dt_fs, w.data(), temperature_K, emin, emax, d_I,
+    return spectrum_core(ctx, d_buf, nprobes, nroi, nframes, nframes, 0, nframes, 1, 1, dt_fs, w.data(), temperature_K, emin, emax, d_I,
                          E_out, nE_out, (cudaStream_t)stream, "tacaw_spectrum");
 }
 
 int tacaw_spectrum_welch(tacaw_ctx* ctx, const void* d_buf, int nprobes, int64_t nroi, int nframes_total, int chunk_len,
-                         int chunk_overlap, double dt_fs, const double* window_table, double temperature_K, double emin,
-                         double emax, float* d_I, double* E_out, int* nE_out, int* nchunks_out, void* stream) {
-    if (!ctx) return TACAW_E_ARG;
-    if (nprobes < 0 || nroi < 0 || nframes_total <= 0 || chunk_len <= 0 || chunk_overlap <= 0 || !(dt_fs > 0) ||
-        !(temperature_K > 0) || !nE_out || !window_table)
+                         int chunk_overlap, int skip_init, int frame_stride, double dt_fs, const double* window_table,
+                         double temperature_K, double emin, double emax, float* d_I, double* E_out, int* nE_out, int* nchunks_out,
+                         void* stream) {
+    TACAW_ENTER(ctx);
+    if (nprobes < 0 || nroi < 0 || nframes_total <= 0 || chunk_len <= 0 || chunk_overlap <= 0 || skip_init < 0 || frame_stride <= 0 ||
+        !(dt_fs > 0) || !(temperature_K > 0) || !nE_out || !window_table)
         return fail(ctx, TACAW_E_ARG, "tacaw_spectrum_welch: bad argument");
-    const int step = chunk_len / chunk_overlap;        // s_{n+1} = s_n + L/nu, remainder-less division
+    // s_{n+1} = s_n + L/nu, remainder-less division, counted in the chunk's own snapshots: with a stride the
+    // next chunk starts (L/nu)*stride stored frames later (reading G24)
+    const long long step = (long long)(chunk_len / chunk_overlap) * frame_stride;
     if (step <= 0) return fail(ctx, TACAW_E_ARG, "tacaw_spectrum_welch: chunk_overlap exceeds chunk_len");
+    const long long span = (long long)(chunk_len - 1) * frame_stride + 1;      // stored frames a chunk covers
     int nchunks = 0;
-    for (int s0 = 0; s0 + chunk_len <= nframes_total; s0 += step) ++nchunks;
+    for (long long s0 = skip_init; s0 + span <= nframes_total; s0 += step) ++nchunks;
     if (nchunks_out) *nchunks_out = nchunks;
-    return spectrum_core(ctx, d_buf, nprobes, nroi, nframes_total, chunk_len, step, nchunks, dt_fs, window_table, temperature_K,
-                         emin, emax, d_I, E_out, nE_out, (cudaStream_t)stream, "tacaw_spectrum_welch");
+    return spectrum_core(ctx, d_buf, nprobes, nroi, nframes_total, chunk_len, skip_init, (int)step, frame_stride, nchunks,
+                         dt_fs * frame_stride, window_table, temperature_K, emin, emax, d_I, E_out, nE_out, (cudaStream_t)stream,
+                         "tacaw_spectrum_welch");
 }
 
 int tacaw_make_scan(int mode, const int32_t* shape, const double* origin, const double* a, const double* b, const double* cell,
@@ -727,7 +892,7 @@ int tacaw_make_detector(const tacaw_grid* g, double lambda, int kind, const doub
 
 int tacaw_detect(tacaw_ctx* ctx, const float* d_I, int nprobes, int nE, int64_t nroi, const float* d_weights, int ndet,
                  float* d_out, void* stream) {
-    if (!ctx) return TACAW_E_ARG;
+    TACAW_ENTER(ctx);
     if (nprobes < 0 || nE < 0 || nroi < 0 || ndet <= 0 || ((nprobes > 0 && nE > 0) && (!d_out || (nroi > 0 && (!d_I || !d_weights)))))
         return fail(ctx, TACAW_E_ARG, "tacaw_detect: bad argument");
     return launch_detect(ctx, d_I, nprobes, nE, nroi, d_weights, ndet, d_out, (cudaStream_t)stream);

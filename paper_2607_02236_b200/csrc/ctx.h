@@ -2,8 +2,11 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <cuda.h>
+
 #include <cstdint>
 #include <string>
+#include <unordered_map>
 #include <vector>
 
 #include "../../include/tacaw.h"
@@ -29,20 +32,27 @@ struct tacaw_ctx {
     float2* d_px = nullptr;  // [nx] exp(-i pi lambda dz h^2/lx^2) / nx
     float2* d_py = nullptr;  // [ny] exp(-i pi lambda dz k^2/ly^2) / ny
 
-    // scratch: metadata region (per-call index arrays) and sort region (build_slices)
-    void* d_meta = nullptr;
-    size_t meta_bytes = 0;
-    void* d_sort = nullptr;
-    size_t sort_bytes = 0;
-    void* d_stage = nullptr;  // staging for the *_host convenience calls
-    size_t stage_bytes = 0;
-    float* d_spec_tab = nullptr;  // window + bose tables
-    size_t spec_tab_bytes = 0;
+    // Workspace: ONE caller-owned device buffer (tacaw_set_workspace), cut into one region per entry point so that
+    // no two entry points share scratch.  The library never allocates device memory after tacaw_create.
+    enum Region { R_BUILD = 0, R_STAGE, R_PROBE, R_PROP, R_ACC, R_SPEC, R_COUNT };
+    char* d_ws = nullptr;
+    size_t ws_bytes = 0;
+    size_t reg_off[R_COUNT] = {0}, reg_bytes[R_COUNT] = {0};
+    int* d_flags = nullptr;       // [4] sticky device-side error flags ([0]: species id out of range), owned by the context
 
     // pinned host arena for per-call index arrays: lets cudaMemcpyAsync return without draining
-    // the stream (a pageable source would synchronise it)
+    // the stream (a pageable source would synchronise it).  Two halves, each guarded by an event recorded
+    // after the last copy issued from it, so reuse waits for exactly those copies.
     char* h_arena = nullptr;
     size_t arena_bytes = 0, arena_off = 0;
+    cudaEvent_t ev_arena[2] = {nullptr, nullptr};
+    bool arena_used[2] = {false, false};
+
+    // per-context (= per-device) kernel state: opt-in shared-memory attribute set / occupancy of each kernel
+    std::unordered_map<const void*, int> kernel_occ;
+    // tensor maps of wave stacks already encoded (key: base pointer, rows, box)
+    struct MapEntry { const void* base; long long rows; int nx, box_cols, box_rows; alignas(64) CUtensorMap tm; };
+    std::vector<MapEntry> maps;
 
     // internal streams: tacaw_propagate runs wave groups round-robin on the caller's stream and these, so one group's
     // kernel tails overlap the other groups' kernels (fork/join with events around the call; TACAW_STREAMS, default 3)
@@ -58,7 +68,25 @@ namespace tacaw {
 
 int fail(tacaw_ctx* ctx, int code, const std::string& msg);
 int cuda_fail(tacaw_ctx* ctx, cudaError_t e, const char* where);
-int ensure(tacaw_ctx* ctx, void** p, size_t* cur, size_t need);
+// region `r` of the caller's workspace if it holds `need` bytes, else TACAW_E_NOMEM (no allocation ever happens here)
+int region(tacaw_ctx* ctx, int r, size_t need, void** out, const char* who);
+// makes ctx->device current for the lifetime of the object and restores the caller's device afterwards
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceGuard(const tacaw_ctx* ctx) {
+        if (cudaGetDevice(&prev) != cudaSuccess) { prev = -1; ok = false; return; }
+        if (prev != ctx->device && cudaSetDevice(ctx->device) != cudaSuccess) ok = false;
+    }
+    ~DeviceGuard() {
+        int cur = -1;
+        if (prev >= 0 && cudaGetDevice(&cur) == cudaSuccess && cur != prev) cudaSetDevice(prev);
+    }
+};
+#define TACAW_ENTER(ctx)                                                   \
+    if (!(ctx)) return TACAW_E_ARG;                                        \
+    tacaw::DeviceGuard guard__(ctx);                                       \
+    if (!guard__.ok) return tacaw::fail(ctx, TACAW_E_CUDA, "cannot make the context's device current")
 // async H2D of a small host array through the pinned arena (falls back to a pageable copy)
 int upload(tacaw_ctx* ctx, void* dst, const void* src, size_t bytes, cudaStream_t st);
 
@@ -97,7 +125,9 @@ struct RowArgs {
 };
 
 struct ColArgs {
-    float2* waves;
+    float2* waves;                 // first wave of this launch
+    float2* stack;                 // the wave stack the tensor map describes (nullptr: `waves` itself) ...
+    int stack_waves, wave0;        //   ... its length and the index of waves[0] in it
     int nwaves, nx;
     int hmax;
     long long nitems;              // (column group, wave) work items; set by the launcher
@@ -113,18 +143,27 @@ struct ColArgs {
 
 int launch_row(tacaw_ctx* ctx, int mode, const RowArgs& a, cudaStream_t st);
 int row_tuple_size(int nx);        // waves per tuple of the row kernel for this grid width
+int slice_step_table_elems(int n); // twiddle table of the slice-step transforms of length n (fft2.cuh XPlan layout) ...
+void slice_step_host_table(int n, float2* tab);   // ... built on the host in fp64
 int launch_col(tacaw_ctx* ctx, int mode, const ColArgs& a, int ny, cudaStream_t st);
 
+// d_nclamped (out): device address of this call's clamp counter inside the build region
 int launch_potential(tacaw_ctx* ctx, const double* d_pos, const int32_t* d_species, int natoms, int nframes, int nspecies,
-                     const AbTable& ab, double dz, int nslices, double z0, float2* d_V, int* d_nclamped,
+                     const AbTable& ab, double dz, int nslices, double z0, float2* d_V, int** d_nclamped,
                      cudaStream_t st);
+// tensor-core K1 (potential_tc.cu): sorted fixed-point coordinates and per-(slice, species) offsets -> V(q) of every slice
+int launch_potential_tc(tacaw_ctx* ctx, const uint32_t* sx, const uint32_t* sy, const int* offsets, int nspecies, const AbTable& ab,
+                        int nslices_total, float2* d_V, cudaStream_t st);
+int potential_tc_max_species();
+constexpr size_t SPEC_TABLE_BYTES = 128 * 1024;     // spectrum region: twiddle/window/Bose tables of one call
 int launch_probe_fill(tacaw_ctx* ctx, const uint32_t* d_uxy /*[P][2] fixed-point fractional*/, int nprobes,
                       const int* d_kap /*[nx]*/, float amp, float2* d_waves, cudaStream_t st);
 int launch_gather(tacaw_ctx* ctx, const float2* d_q, int nwaves, const int* d_wp, const int* d_wf, const int* d_idx,
                   int64_t nroi, float2* d_buf, int nprobes, int nframes, cudaStream_t st);
-// probe_stride: elements between the series blocks of consecutive probes; accumulate: add to d_I instead of storing
+// probe_stride / frame_stride / chunk_stride: elements between consecutive probes' series blocks, consecutive frames of a
+// chunk, and the first frames of consecutive Welch chunks; all nchunks chunks are transformed and summed in one launch
 int launch_spectrum(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int64_t nroi, int nframes, size_t probe_stride,
-                    int accumulate, const float2* d_roots,
+                    size_t frame_stride, int nchunks, size_t chunk_stride, const float2* d_roots,
                     const float* d_window, const float* d_bose, int e_lo, int nE, float* d_I, cudaStream_t st);
 
 int launch_detect(tacaw_ctx* ctx, const float* d_I, int nprobes, int nE, int64_t nroi, const float* d_w, int ndet, float* d_out,

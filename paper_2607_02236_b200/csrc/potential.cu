@@ -8,6 +8,8 @@
 // three quadrants follow from the same four real sums (see k_potential).
 // Phases use fixed-point fractional coordinates U = round(u 2^32): (h*U mod 2^32) is exact
 // integer arithmetic, then sincospif -- fp32 h*x/L would lose ~4e-4 rad at |h| ~ 1000.
+#include <cstdlib>
+
 #include "ctx.h"
 
 namespace tacaw {
@@ -17,7 +19,7 @@ namespace tacaw {
 __global__ void k_atom_keys(const double* __restrict__ pos, const int32_t* __restrict__ species, int natoms,
                             long long ntotal, int nspecies, double dz, int nslices, double z0, double inv_lx,
                             double inv_ly, int* __restrict__ keys, uint32_t* __restrict__ ux, uint32_t* __restrict__ uy,
-                            int* __restrict__ counts, int* __restrict__ nclamped) {
+                            int* __restrict__ counts, int* __restrict__ nclamped, int* __restrict__ flags) {
     long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= ntotal) return;
     const int f = (int)(i / natoms), j = (int)(i - (long long)f * natoms);
@@ -27,7 +29,7 @@ __global__ void k_atom_keys(const double* __restrict__ pos, const int32_t* __res
     else if (fz > (double)(nslices - 1)) { n = nslices - 1; atomicAdd(nclamped, 1); }
     else n = (int)fz;
     int s = species[j];
-    if (s < 0 || s >= nspecies) { atomicAdd(nclamped + 1, 1); s = 0; }
+    if (s < 0 || s >= nspecies) { atomicAdd(flags, 1); s = 0; }     // sticky: reported by tacaw_device_status
     int key = (f * nslices + n) * nspecies + s;
     keys[i] = key;
     atomicAdd(counts + key, 1);
@@ -230,19 +232,22 @@ __global__ void __launch_bounds__(POT_THREADS) k_potential(const uint32_t* __res
 }
 
 int launch_potential(tacaw_ctx* ctx, const double* d_pos, const int32_t* d_species, int natoms, int nframes, int nspecies,
-                     const AbTable& ab, double dz, int nslices, double z0, float2* d_V, int* d_nclamped,
+                     const AbTable& ab, double dz, int nslices, double z0, float2* d_V, int** d_nclamped_out,
                      cudaStream_t st) {
     const int nx = ctx->grid.nx, ny = ctx->grid.ny;
     const long long ntotal = (long long)natoms * nframes;
     const long long nkeys_ll = (long long)nframes * nslices * nspecies;
     if (nkeys_ll > (1LL << 30) || ntotal > (1LL << 31) - 1) return fail(ctx, TACAW_E_UNSUPPORTED, "batch too large");
     const int nkeys = (int)nkeys_ll;
-    // sort scratch layout: keys[nt] ux[nt] uy[nt] sx[nt] sy[nt] counts[nkeys] offsets[nkeys+1]
+    // build region layout: clamp counter (256 B) | keys[nt] ux[nt] uy[nt] sx[nt] sy[nt] counts[nkeys] offsets[nkeys+1]
     size_t nt = (size_t)(ntotal > 0 ? ntotal : 1);
-    size_t need = sizeof(int) * (5 * nt + 2 * (size_t)nkeys + 2);
-    int rc = ensure(ctx, &ctx->d_sort, &ctx->sort_bytes, need);
+    size_t need = 256 + sizeof(int) * (5 * nt + 2 * (size_t)nkeys + 2);
+    void* reg = nullptr;
+    int rc = region(ctx, tacaw_ctx::R_BUILD, need, &reg, "tacaw_build_slices");
     if (rc) return rc;
-    int* keys = (int*)ctx->d_sort;
+    int* d_nclamped = (int*)reg;
+    *d_nclamped_out = d_nclamped;
+    int* keys = (int*)((char*)reg + 256);
     uint32_t* ux = (uint32_t*)(keys + nt);
     uint32_t* uy = ux + nt;
     uint32_t* sx = uy + nt;
@@ -250,13 +255,13 @@ int launch_potential(tacaw_ctx* ctx, const double* d_pos, const int32_t* d_speci
     int* counts = (int*)(sy + nt);
     int* offsets = counts + nkeys;
     TACAW_CUDA(ctx, cudaMemsetAsync(counts, 0, sizeof(int) * (2 * (size_t)nkeys + 1), st));
-    TACAW_CUDA(ctx, cudaMemsetAsync(d_nclamped, 0, 2 * sizeof(int), st));
+    TACAW_CUDA(ctx, cudaMemsetAsync(d_nclamped, 0, sizeof(int), st));
     // d_V is not cleared: k_potential writes every in-band (h,k), and the column pass that follows reads only those
     if (ntotal == 0) TACAW_CUDA(ctx, cudaMemsetAsync(d_V, 0, sizeof(float2) * (size_t)nframes * nslices * nx * ny, st));
     if (ntotal > 0) {
         k_atom_keys<<<(unsigned)((ntotal + 255) / 256), 256, 0, st>>>(d_pos, d_species, natoms, ntotal, nspecies, dz, nslices,
                                                                      z0, 1.0 / ctx->grid.lx_A, 1.0 / ctx->grid.ly_A, keys, ux,
-                                                                     uy, counts, d_nclamped);
+                                                                     uy, counts, d_nclamped, ctx->d_flags);
         ctx->launches++;
     }
     k_scan_counts<<<1, 1024, 0, st>>>(counts, nkeys, offsets);
@@ -267,6 +272,11 @@ int launch_potential(tacaw_ctx* ctx, const double* d_pos, const int32_t* d_speci
         ctx->launches++;
         const int hmax = ctx->hmax_pot;
         const int total_slices = nframes * nslices;
+        // K1 on the tensor cores (potential_tc.cu) unless TACAW_K1_TC=0 asks for the fp32-pipe kernel below (kept for
+        // comparison and for more than four species)
+        static const bool use_tc = [] { const char* e = getenv("TACAW_K1_TC"); return e ? atoi(e) != 0 : true; }();
+        if (use_tc && nspecies <= potential_tc_max_species())
+            return launch_potential_tc(ctx, sx, sy, offsets, nspecies, ab, total_slices, d_V, st);
         for (int z0i = 0; z0i < total_slices; z0i += 65535) {
             int nz = total_slices - z0i < 65535 ? total_slices - z0i : 65535;
             dim3 grid((hmax + 1 + POT_T - 1) / POT_T, (ctx->kmaxmax_pot + 1 + POT_T - 1) / POT_T, nz);

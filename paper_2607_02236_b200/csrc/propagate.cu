@@ -22,6 +22,22 @@
 #include "ctx.h"
 #include "fft2.cuh"
 
+// 2048-point row kernel: teams (rows in flight) per CTA, and where the 8 KB combine table of the pair plan lives.
+// 2 teams + table in global memory (read through L1): 74.5 KB per CTA, three CTAs = 12 warps per SM
+#ifndef TACAW_ROW2048_TEAMS
+#define TACAW_ROW2048_TEAMS 2
+#endif
+#ifndef TACAW_COL2048_MERGE
+#define TACAW_COL2048_MERGE 0
+#endif
+#ifndef TACAW_ROW2048_CW_SMEM
+#define TACAW_ROW2048_CW_SMEM 0
+#endif
+// combine twiddles of the row kernel computed from w^kq and compile-time constants instead of read from the table
+#ifndef TACAW_ROW2048_CW_COMPUTE
+#define TACAW_ROW2048_CW_COMPUTE 1
+#endif
+
 namespace tacaw {
 
 // Which of a thread's elements x[tid + T*m] are inside the band |h| <= H (index <= H or >= N - H).
@@ -50,16 +66,22 @@ struct Band {
 // ------------------------------------------------------------------------------------------
 template <int N>
 struct RowCfg {
-    using P = Plan2<N>;
-    static constexpr int E = P::E, T = P::T;
+    using X = XPlan<N>;
+    static constexpr int E = X::E, T = X::T;
     static constexpr int TEAM = (T < 32) ? 32 : T;          // threads that share an exchange buffer
     static constexpr int RPT = TEAM / T;                    // rows (one per wave of a tuple) a team transforms at once
-    static constexpr int TEAMS = (N >= 2048) ? 2 : 4;       // teams per CTA
+    static constexpr int TEAMS = (N >= 2048) ? TACAW_ROW2048_TEAMS : 4;       // teams per CTA
     static constexpr int THREADS = TEAMS * TEAM;
-    static constexpr int XE = exch2_elems(N, 1);            // exchange elements per row
+    static constexpr int XE = X::exch(1);                   // exchange elements per row
     static constexpr int MINB = (N >= 2048) ? 1 : 3;
+    static constexpr bool CW_SMEM = !X::PAIR || (TACAW_ROW2048_CW_SMEM != 0);
+    static constexpr int TW = CW_SMEM ? X::TW_ELEMS : X::P::TW_ELEMS;     // twiddle entries held in shared memory
+    // staged t_n row: in the paired ownership a lane pair reads elements 512 apart, i.e. the same banks; every block of 512
+    // elements is therefore shifted by 8 more elements (16 banks), which keeps the half-warp wavefronts conflict free
+    static constexpr int TROW = X::PAIR ? N + 8 * (N / 512) : N;
+    static constexpr __host__ __device__ int tskew(int i) { return X::PAIR ? i + 8 * (i >> 9) : i; }
     static constexpr size_t smem(bool has_t) {
-        return sizeof(float2) * ((size_t)P::TW_ELEMS + (size_t)TEAMS * (RPT * XE + (has_t ? N : 0)));
+        return sizeof(float2) * ((size_t)TW + (size_t)TEAMS * (RPT * XE + (has_t ? TROW : 0)));
     }
 };
 
@@ -74,7 +96,7 @@ struct RowCfg {
 template <int N, int MODE, bool BAND>
 __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MINB) k_row(RowArgs a) {
     using C = RowCfg<N>;
-    using P = Plan2<N>;
+    using X = XPlan<N>;
     constexpr int E = C::E, T = C::T, TEAM = C::TEAM, RPT = C::RPT;
     constexpr bool HAS_T = (MODE == ROW_FIRST || MODE == ROW_MID);
     constexpr bool FULL_IN = (MODE == ROW_FIRST);           // the input row is an r-space row: no band
@@ -83,12 +105,12 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MINB) k_row(Row
     const int team = lt / TEAM, l = lt % TEAM;
     const int g = l / T, tid = l % T;
     float2* tw = smem;
-    float2* exw = smem + P::TW_ELEMS + (size_t)team * (RPT * C::XE + (HAS_T ? N : 0));   // team's exchange rows
+    float2* exw = smem + C::TW + (size_t)team * (RPT * C::XE + (HAS_T ? C::TROW : 0));   // team's exchange rows
     float2* ex = exw + (size_t)g * C::XE;
     float2* sT = exw + (size_t)RPT * C::XE;                                              // [N]
     pdl_launch_dependents();
-    fft2_load_twiddles<N>(tw, a.roots, lt, C::THREADS);
-    const float2* twp = tw + tid;
+    xplan_load_twiddles<N, C::CW_SMEM>(tw, a.roots, lt, C::THREADS);
+    const XThread<N, 1, X::PAIR && (TACAW_ROW2048_CW_COMPUTE != 0)> xt(tw, C::CW_SMEM ? tw + X::P::TW_ELEMS : a.roots + X::P::TW_ELEMS, tid, 0);
     const Band<N, T, BAND> band(tid, a.hmax);
 
     const long long gteam = (long long)blockIdx.x * C::TEAMS + team;
@@ -172,12 +194,13 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MINB) k_row(Row
         }
         cp_async_commit();
     };
+    const unsigned long long pol_t = l2_policy_evict_first();     // t_n is read once per group: do not keep it in L2
     auto issue_t = [&](int f, int yv) {
         const float2* tp = a.trans[(size_t)f * a.nseg + a.seg] + (size_t)a.slice * npix + (size_t)yv * N;
         constexpr int KT = (N / 2 + TEAM - 1) / TEAM;
 #pragma unroll
         for (int j = 0; j < KT; ++j)
-            if (N / 2 >= TEAM * KT || l + TEAM * j < N / 2) cp_async16(sT + 2 * (l + TEAM * j), tp + 2 * (l + TEAM * j));
+            if (N / 2 >= TEAM * KT || l + TEAM * j < N / 2) cp_async16_hint(sT + C::tskew(2 * (l + TEAM * j)), tp + 2 * (l + TEAM * j), pol_t);
         cp_async_commit();
     };
 
@@ -226,7 +249,7 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MINB) k_row(Row
             float2 x[E];
 #pragma unroll
             for (int m = 0; m < E; ++m) {
-                if (FULL_IN) x[m] = ex[tid + T * m];
+                if (FULL_IN) x[m] = ex[xt.mid(m)];          // r-space row, straight into the second transform
                 else if (Band<N, T, BAND>::never(m)) x[m] = make_float2(0.f, 0.f);
                 else x[m] = band.in(m, tid) ? ex[tid + T * m] : make_float2(0.f, 0.f);
             }
@@ -249,19 +272,23 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MINB) k_row(Row
             };
             auto nopre = []() {};
             Hooks<decltype(nopre), decltype(post)> hook{nopre, post};
+            NoHook nohook;
             if constexpr (MODE != ROW_FIRST) {
-                if constexpr (HAS_T) fft2<N, 1, true, true>(x, twp, ex, tid, 0, sync);
-                else fft2<N, 1, true, true>(x, twp, ex, tid, 0, sync, hook);
+                if constexpr (HAS_T) xt.template first<true, true>(x, ex, sync, nohook);
+                else xt.template first<true, true>(x, ex, sync, hook);
             }
+            // between the transforms register m holds element xt.mid(m) of the row (== tid + T m except at 2048)
+            float2* wmid = a.waves + (size_t)wv * npix + (size_t)y * N + xt.mid0;
             if constexpr (HAS_T) {
                 if (t_new && i > i0) {
                     cp_async_wait_all();
                     sync();
                 }
-                const float2* st = sT + tid;
+                // (mid0 < 1024 and mid_off is a multiple of 32: the skews of base and offset add up)
+                const float2* st = sT + C::tskew(xt.mid0);
 #pragma unroll
-                for (int m = 0; m < E; ++m) x[m] = cmul(x[m], st[T * m]);
-                fft2<N, 1, false, true>(x, twp, ex, tid, 0, sync, hook);
+                for (int m = 0; m < E; ++m) x[m] = cmul(x[m], st[C::tskew(xt.mid_off(m))]);
+                xt.template second<false, true>(x, ex, sync, hook);
 #pragma unroll
                 for (int m = 0; m < E; ++m) {
                     if (!Band<N, T, BAND>::never(m)) {
@@ -270,13 +297,13 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MINB) k_row(Row
                 }
             } else if constexpr (MODE == ROW_LAST) {
 #pragma unroll
-                for (int m = 0; m < E; ++m) wrow[T * m] = x[m];
+                for (int m = 0; m < E; ++m) wmid[xt.mid_off(m)] = x[m];
             } else {  // ROW_TRANS: t = exp(i sigma v), v = Re(x)/(lx ly)
 #pragma unroll
                 for (int m = 0; m < E; ++m) {
                     float s, c;
                     sincosf(a.scale * x[m].x, &s, &c);
-                    wrow[T * m] = make_float2(c, s);
+                    wmid[xt.mid_off(m)] = make_float2(c, s);
                 }
             }
             p = pn;
@@ -309,16 +336,20 @@ static cudaError_t launch_pdl(K kern, unsigned grid, int threads, size_t smem, c
     return cudaLaunchKernelEx(&cfg, kern, a...);
 }
 
-// grid that fills the machine exactly: occupancy x SM count CTAs
+// grid that fills the machine exactly: occupancy x SM count CTAs.  The opt-in shared-memory attribute and the occupancy
+// are per device: cached on the context (one context = one device), keyed by the kernel.
 template <class K>
-static int machine_ctas(const tacaw_ctx* ctx, K kern, int threads, size_t smem, int* cache) {
-    if (*cache == 0) {
+static int machine_ctas(tacaw_ctx* ctx, K kern, int threads, size_t smem, int* out) {
+    const void* key = (const void*)kern;
+    auto it = ctx->kernel_occ.find(key);
+    if (it == ctx->kernel_occ.end()) {
+        if (smem > 48 * 1024) TACAW_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         int per_sm = 0;
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem) != cudaSuccess || per_sm < 1) {
             (void)cudaGetLastError();
             per_sm = 1;
         }
-        *cache = per_sm;
+        it = ctx->kernel_occ.emplace(key, per_sm).first;
     }
     // TACAW_GRID_FRAC (tuning knob, default 1): launch only this fraction of the machine-filling grid, so that kernels of
     // different streams share the machine side by side instead of one after the other
@@ -327,8 +358,9 @@ static int machine_ctas(const tacaw_ctx* ctx, K kern, int threads, size_t smem, 
         const double v = e ? atof(e) : 1.0;
         return (v > 0.0 && v <= 1.0) ? v : 1.0;
     }();
-    const int n = (int)(ctx->num_sms * (*cache) * frac);
-    return n < 1 ? 1 : n;
+    const int n = (int)(ctx->num_sms * it->second * frac);
+    *out = n < 1 ? 1 : n;
+    return TACAW_OK;
 }
 
 template <int N, int MODE, bool BAND>
@@ -338,14 +370,10 @@ static int launch_row_nb(tacaw_ctx* ctx, const RowArgs& a0, cudaStream_t st) {
     if (!a.tuples) a.ntuples = (a.nwaves + C::RPT - 1) / C::RPT;
     const size_t smem = C::smem(MODE == ROW_FIRST || MODE == ROW_MID);
     auto kern = k_row<N, MODE, BAND>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (smem > 48 * 1024) TACAW_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
-    }
-    static int occ_cache = 0;
     a.nitems = (long long)a.ny * a.ntuples;
-    long long teams = (long long)machine_ctas(ctx, kern, C::THREADS, smem, &occ_cache) * C::TEAMS;
+    int mctas = 0;
+    if (int rc = machine_ctas(ctx, kern, C::THREADS, smem, &mctas)) return rc;
+    long long teams = (long long)mctas * C::TEAMS;
     if (teams > a.nitems) teams = a.nitems;
     a.ipc = (int)((a.nitems + teams - 1) / teams);
     teams = (a.nitems + a.ipc - 1) / a.ipc;
@@ -379,6 +407,9 @@ int row_tuple_size(int nx) {
     return t < 32 ? 32 / t : 1;
 }
 
+int slice_step_table_elems(int n) { return xplan_table_elems(n); }
+void slice_step_host_table(int n, float2* tab) { xplan_host_table(n, tab); }
+
 int launch_row(tacaw_ctx* ctx, int mode, const RowArgs& a, cudaStream_t st) {
     if (a.nwaves <= 0) return TACAW_OK;
     switch (ctx->grid.nx) {
@@ -397,52 +428,59 @@ int launch_row(tacaw_ctx* ctx, int mode, const RowArgs& a, cudaStream_t st) {
 // ------------------------------------------------------------------------------------------
 template <int N, int MODE = COL_MID>
 struct ColCfg {
-    using P = Plan2<N>;
-    static constexpr int E = P::E, T = P::T;
+    using X = XPlan<N>;
+    static constexpr int E = X::E, T = X::T;
     // adjacent columns transformed together.  The slice step reads its tiles from L2, where 64-byte row segments are
     // full speed; the potential pass (COL_INV at 256^2 and below) streams from HBM, where they cost a 2x over-fetch
     // (ncu: 7.4 GB read for 3.7 GB of tiles), so it takes full 128-byte lines
     static constexpr int WC = (N >= 1024) ? 4 : ((MODE == COL_INV && N <= 256) ? 16 : 8);
     static constexpr bool PY_SMEM = (N <= 512);              // Py table in shared memory (else read through L1)
     static constexpr int THREADS = T * WC;
-    static constexpr int XE = exch2_elems(N, WC);
-    static constexpr int MINB = (N <= 1024) ? 3 : 1;
+    static constexpr int XE = X::exch(WC);
+    // MERGE (2048): the TMA staging tile and the exchange buffer are ONE region (a tile is in registers before the first
+    // exchange is written, and the next tile is requested only after the last exchange of the item has been read back):
+    // 84 KB instead of 148 KB per CTA, so two CTAs (16 warps) fit an SM
+    static constexpr bool MERGE = X::PAIR && (TACAW_COL2048_MERGE != 0);
+    static constexpr int MINB = (N <= 1024) ? 3 : (MERGE ? 2 : 1);
     // twiddles | Py | (pad to 128 B) staging tile [N][WC] (TMA destination) | exchange | mbarrier
-    static constexpr int OFF_S = ((P::TW_ELEMS + (PY_SMEM ? N : 0)) + 15) / 16 * 16;
+    static constexpr int OFF_S = ((X::TW_ELEMS + (PY_SMEM ? N : 0)) + 15) / 16 * 16;
     static constexpr int RB = (N < 256) ? N : 256;            // rows per TMA box
-    static constexpr size_t smem() { return sizeof(float2) * ((size_t)OFF_S + (size_t)N * WC + XE + 2); }
+    static constexpr int OFF_X = OFF_S + (MERGE ? 0 : N * WC);
+    static_assert(!MERGE || XE >= N * WC, "merged region must hold a tile");
+    static constexpr size_t smem() { return sizeof(float2) * ((size_t)OFF_X + XE + 2); }
 };
 
 // Work items of a column launch are (column group, wave) pairs, flattened as gi*nwaves + w over the
 // selected groups (the in-band ones, or all of them when hmax covers the grid) and dealt out in equal
 // contiguous ranges to a machine-filling grid, like the row kernel.  The [N][WC] tile of the NEXT item is
-// prefetched with cp.async into a staging buffer while the current one is transformed.
+// staged by TMA while the current one is transformed.
 // BAND: every kmax[ix] <= N/3, so the chunks of k strictly between N/3 and N - N/3 are masked for
-// every column and are neither multiplied nor tested.
+// every column and are neither multiplied nor tested (single-exchange plans; the pair plan tests every element).
 template <int N, int MODE, bool BAND>
 __global__ void __launch_bounds__(ColCfg<N, MODE>::THREADS, ColCfg<N, MODE>::MINB) k_col(ColArgs a, const __grid_constant__ CUtensorMap tm) {
     using C = ColCfg<N, MODE>;
-    using P = Plan2<N>;
+    using X = XPlan<N>;
     constexpr int E = C::E, T = C::T, WC = C::WC;
+    constexpr bool MERGE = C::MERGE;
     extern __shared__ __align__(128) float2 smem[];
     const int lt = threadIdx.x;
     const int c = lt % WC, tid = lt / WC;
     float2* tw = smem;
-    float2* sPy = smem + P::TW_ELEMS;             // Py[ky]
+    float2* sPy = smem + X::TW_ELEMS;             // Py[ky]
     float2* sS = smem + C::OFF_S;                 // staging tile
-    float2* ex = sS + N * WC;
+    float2* ex = smem + C::OFF_X;                 // exchange buffer (the same region when MERGE)
     unsigned long long* bar = reinterpret_cast<unsigned long long*>(ex + C::XE);
     pdl_launch_dependents();
     if (lt == 0) {
         mbar_init(bar, 1);
         mbar_init_fence();
     }
-    fft2_load_twiddles<N>(tw, a.roots, lt, C::THREADS);
+    xplan_load_twiddles<N>(tw, a.roots, lt, C::THREADS);
     if constexpr (MODE != COL_INV && C::PY_SMEM) {
         for (int i = lt; i < N / 2; i += C::THREADS) cp_async16(sPy + 2 * i, a.py + 2 * i);
         cp_async_commit();
     }
-    const float2* twp = tw + tid;
+    const XThread<N, WC> xt(tw, tw + X::P::TW_ELEMS, tid, c);
     const int NG = a.nx / WC;
     const int nlo = a.hmax / WC + 1;            // groups covering ix in [0, hmax]
     const int nhi = (a.hmax + WC - 1) / WC;     // groups covering ix in [nx-hmax, nx)
@@ -451,7 +489,7 @@ __global__ void __launch_bounds__(ColCfg<N, MODE>::THREADS, ColCfg<N, MODE>::MIN
     const long long i0 = (long long)blockIdx.x * a.ipc;
     const long long i1 = min(i0 + (long long)a.ipc, a.nitems);
     const size_t npix = (size_t)N * a.nx;
-    using B = Band<N, T, BAND>;
+    using B = Band<N, T, BAND && !X::PAIR>;
     // tile of wave wv, column group grp -> staging: one TMA box of [RB rows][WC columns] per RB rows, issued by one
     // thread, completion counted in bytes on the mbarrier (every thread has passed a barrier after its last read of sS)
     auto issue_tile = [&](int wv, int grp) {
@@ -459,7 +497,7 @@ __global__ void __launch_bounds__(ColCfg<N, MODE>::THREADS, ColCfg<N, MODE>::MIN
             fence_proxy_async();
             mbar_expect_tx(bar, (unsigned)(N * WC * sizeof(float2)));
 #pragma unroll
-            for (int b = 0; b < N / C::RB; ++b) tma_load_2d(sS + b * C::RB * WC, &tm, grp * WC, wv * N + b * C::RB, bar);
+            for (int b = 0; b < N / C::RB; ++b) tma_load_2d(sS + b * C::RB * WC, &tm, grp * WC, (a.wave0 + wv) * N + b * C::RB, bar);
         }
     };
     unsigned parity = 0;
@@ -477,17 +515,19 @@ __global__ void __launch_bounds__(ColCfg<N, MODE>::THREADS, ColCfg<N, MODE>::MIN
         if (i0 >= i1) return;
         int cur_gi = -1;
         float2 px = make_float2(0.f, 0.f);
+        int km = -1;
         int dlo = -1, dhi = -1;                  // |k| <= km  <=>  T*m <= dlo (m < E/2)  or  N - T*m <= dhi (m >= E/2)
         bool live = true;
-        size_t coloff = 0;
+        size_t coloff = 0, midoff = 0;
         for (long long i = i0; i < i1; ++i) {
             if (gi != cur_gi) {
                 cur_gi = gi;
                 const int ix = group_of(gi) * WC + c;
                 coloff = (size_t)ix + (size_t)tid * a.nx;
+                midoff = (size_t)ix + (size_t)xt.mid0 * a.nx;
                 // a column entirely outside the mask is never written by the row kernel: it is not
                 // used (NaN * 0 would not be 0) and comes out as zeros
-                const int km = a.kmax[ix];
+                km = a.kmax[ix];
                 live = km >= 0;
                 dlo = km - tid;
                 dhi = km + tid;
@@ -496,7 +536,17 @@ __global__ void __launch_bounds__(ColCfg<N, MODE>::THREADS, ColCfg<N, MODE>::MIN
                     px = make_float2(px.x * a.pscale, px.y * a.pscale);
                 }
             }
+            // |k| <= km for the element register m holds BETWEEN the transforms (row xt.mid(m) of the column)
+            auto keep_mid = [&](int m) {
+                if constexpr (X::PAIR) {
+                    const int r = xt.mid0 + pair_off(m & 15);            // row in the lower half
+                    return (m < 16) ? (r <= km) : (N / 2 - r <= km);      // row r + N/2 is k = r - N/2
+                } else {
+                    return (T * m < N / 2) ? (T * m <= dlo) : (N - T * m <= dhi);
+                }
+            };
             float2* wc = a.waves + (size_t)w * npix + coloff;
+            float2* wmid = a.waves + (size_t)w * npix + midoff;
             const size_t rs = (size_t)T * a.nx;
             mbar_wait(bar, parity);              // this item's tile has landed
             parity ^= 1;
@@ -511,24 +561,46 @@ __global__ void __launch_bounds__(ColCfg<N, MODE>::THREADS, ColCfg<N, MODE>::MIN
             if (wn == a.nwaves) { wn = 0; ++gn; }
             const bool more = (i + 1 < i1);
             sync();                              // staging tile consumed; previous exchange read back
-            if (more) issue_tile(wn, group_of(gn));
-            if constexpr (MODE != COL_INV) {
-                fft2<N, WC, false, false>(x, twp, ex, tid, c, sync);
+            if constexpr (!MERGE) {
+                if (more) issue_tile(wn, group_of(gn));
+            }
+            // MERGE: the next tile goes into the exchange region, as soon as the item's last exchange has been read back
+            auto nopre = []() {};
+            auto post = [&]() {
+                if constexpr (MERGE) {
+                    if (more) {
+                        sync();
+                        issue_tile(wn, group_of(gn));
+                    }
+                }
+            };
+            Hooks<decltype(nopre), decltype(post)> hook{nopre, post};
+            NoHook nohook;
+            if constexpr (MODE == COL_INV) {
+                xt.template first<true, false>(x, ex, sync, hook);
+#pragma unroll
+                for (int m = 0; m < E; ++m) wmid[(size_t)xt.mid_off(m) * a.nx] = x[m];
+            } else {
+                if constexpr (MODE == COL_LASTQ) xt.template first<false, false>(x, ex, sync, hook);
+                else xt.template first<false, false>(x, ex, sync, nohook);
 #pragma unroll
                 for (int m = 0; m < E; ++m) {
                     if (B::never(m)) {
                         x[m] = make_float2(0.f, 0.f);
                     } else {
-                        const bool keep = (T * m < N / 2) ? (T * m <= dlo) : (N - T * m <= dhi);
-                        const float2 p = cmul(px, C::PY_SMEM ? sPy[tid + T * m] : __ldg(a.py + tid + T * m));
-                        x[m] = keep ? cmul(x[m], p) : make_float2(0.f, 0.f);
+                        const float2 p = cmul(px, C::PY_SMEM ? sPy[xt.mid(m)] : __ldg(a.py + xt.mid(m)));
+                        x[m] = keep_mid(m) ? cmul(x[m], p) : make_float2(0.f, 0.f);
                     }
                 }
-            }
-            if constexpr (MODE == COL_MID) fft2<N, WC, true, true>(x, twp, ex, tid, c, sync);
-            else if constexpr (MODE == COL_INV) fft2<N, WC, true, false>(x, twp, ex, tid, c, sync);
+                if constexpr (MODE == COL_MID) {
+                    xt.template second<true, true>(x, ex, sync, hook);
 #pragma unroll
-            for (int m = 0; m < E; ++m) wc[m * rs] = x[m];
+                    for (int m = 0; m < E; ++m) wc[m * rs] = x[m];
+                } else {
+#pragma unroll
+                    for (int m = 0; m < E; ++m) wmid[(size_t)xt.mid_off(m) * a.nx] = x[m];
+                }
+            }
             w = wn;
             gi = gn;
         }
@@ -563,6 +635,21 @@ static int make_tile_map(tacaw_ctx* ctx, CUtensorMap* tm, const void* base, int 
     return TACAW_OK;
 }
 
+// Tensor maps are encoded once per wave stack and kept on the context (cuTensorMapEncodeTiled per launch costs host time on
+// a path that issues one launch every few microseconds); a small FIFO, cleared when the workspace changes.
+static int tile_map(tacaw_ctx* ctx, const CUtensorMap** out, const void* base, int nx, long long rows, int box_cols, int box_rows) {
+    for (auto& e : ctx->maps)
+        if (e.base == base && e.rows == rows && e.nx == nx && e.box_cols == box_cols && e.box_rows == box_rows) { *out = &e.tm; return TACAW_OK; }
+    if (ctx->maps.size() >= 16) ctx->maps.erase(ctx->maps.begin());
+    ctx->maps.emplace_back();
+    auto& e = ctx->maps.back();
+    e.base = base; e.rows = rows; e.nx = nx; e.box_cols = box_cols; e.box_rows = box_rows;
+    int rc = make_tile_map(ctx, &e.tm, base, nx, rows, box_cols, box_rows);
+    if (rc) { ctx->maps.pop_back(); return rc; }
+    *out = &e.tm;
+    return TACAW_OK;
+}
+
 // zero the out-of-band columns [c0, c1) of every row of every wave (exit wave Psi_S, O7)
 __global__ void k_zero_cols(float2* __restrict__ waves, long long nrows, int nx, int c0, int c1) {
     const int width = (c1 - c0) / 2;      // float4 = two complex values; c0, c1 are even
@@ -584,23 +671,18 @@ static int launch_col_nb(tacaw_ctx* ctx, const ColArgs& a0, cudaStream_t st) {
     const int ngroups = all ? NG : nlo + nhi;
     const size_t smem = C::smem();
     auto kern = k_col<N, MODE, BAND>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (smem > 48 * 1024) TACAW_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
-    }
-    static int occ_cache = 0;
     a.nitems = (long long)ngroups * a.nwaves;
-    long long ctas = machine_ctas(ctx, kern, C::THREADS, smem, &occ_cache);
+    int mctas = 0;
+    if (int rc = machine_ctas(ctx, kern, C::THREADS, smem, &mctas)) return rc;
+    long long ctas = mctas;
     if (ctas > a.nitems) ctas = a.nitems;
     a.ipc = (int)((a.nitems + ctas - 1) / ctas);
     ctas = (a.nitems + a.ipc - 1) / a.ipc;
-    alignas(64) CUtensorMap tm;
-    {
-        int rc = make_tile_map(ctx, &tm, a.waves, a.nx, (long long)a.nwaves * N, C::WC, C::RB);
-        if (rc) return rc;
-    }
-    TACAW_CUDA(ctx, launch_pdl(kern, (unsigned)ctas, C::THREADS, smem, st, a.pdl != 0, a, tm));
+    // one tensor map per wave stack (not per launch): the launch addresses its waves by their index in the stack
+    if (!a.stack) { a.stack = a.waves; a.stack_waves = a.nwaves; a.wave0 = 0; }
+    const CUtensorMap* tmp = nullptr;
+    if (int rc = tile_map(ctx, &tmp, a.stack, a.nx, (long long)a.stack_waves * N, C::WC, C::RB)) return rc;
+    TACAW_CUDA(ctx, launch_pdl(kern, (unsigned)ctas, C::THREADS, smem, st, a.pdl != 0, a, *tmp));
     ctx->launches++;
     if (MODE == COL_LASTQ && !all) {
         const int c0 = nlo * C::WC, c1 = (NG - nhi) * C::WC;

@@ -26,8 +26,8 @@ struct SpecCfg {
 
 template <int N>
 __global__ void __launch_bounds__(SpecCfg<N>::THREADS) k_spectrum(const float2* __restrict__ buf, long long nroi,
-                                                                  size_t probe_stride, int accumulate,
-                                                                  const float2* __restrict__ roots,
+                                                                  size_t probe_stride, size_t frame_stride, int nchunks,
+                                                                  size_t chunk_stride, const float2* __restrict__ roots,
                                                                   const float* __restrict__ window,
                                                                   const float* __restrict__ bose, int e_lo, int nE,
                                                                   float* __restrict__ I) {
@@ -55,20 +55,31 @@ __global__ void __launch_bounds__(SpecCfg<N>::THREADS) k_spectrum(const float2* 
     const long long r = (long long)blockIdx.x * WQ + c;
     const bool live = r < nroi;
     const float2* src = buf + (size_t)p * probe_stride + (live ? r : 0);
-    float2 x[E];
+    // Welch chunks (Eq.(2)): every chunk of the series is transformed here and |Phi|^2 summed in registers, so I is
+    // written once (bose[] carries the 1/N of the average)
+    float acc[E];
 #pragma unroll
-    for (int m = 0; m < E; ++m) {
-        int f = tid + T * m;
-        float2 v = live ? src[(size_t)f * nroi] : make_float2(0.f, 0.f);
-        float w = window[f];
-        x[m] = make_float2(v.x * w, v.y * w);
-    }
-    if constexpr (C::THREADS <= 32) {
-        SyncWarp sync;
-        fft_regs<N, E, WQ, false, TWREG>(x, tw, roots_s, smA, smB, tid, c, sync);
-    } else {
-        SyncBlock sync;
-        fft_regs<N, E, WQ, false, TWREG>(x, tw, roots_s, smA, smB, tid, c, sync);
+    for (int m = 0; m < E; ++m) acc[m] = 0.f;
+    for (int ch = 0; ch < nchunks; ++ch, src += chunk_stride) {
+        float2 x[E];
+#pragma unroll
+        for (int m = 0; m < E; ++m) {
+            int f = tid + T * m;
+            float2 v = live ? src[(size_t)f * frame_stride] : make_float2(0.f, 0.f);
+            float w = window[f];
+            x[m] = make_float2(v.x * w, v.y * w);
+        }
+        if constexpr (C::THREADS <= 32) {
+            SyncWarp sync;
+            if (ch > 0) sync();
+            fft_regs<N, E, WQ, false, TWREG>(x, tw, roots_s, smA, smB, tid, c, sync);
+        } else {
+            SyncBlock sync;
+            if (ch > 0) sync();                         // the previous chunk's last exchange has been read back
+            fft_regs<N, E, WQ, false, TWREG>(x, tw, roots_s, smA, smB, tid, c, sync);
+        }
+#pragma unroll
+        for (int m = 0; m < E; ++m) acc[m] += x[m].x * x[m].x + x[m].y * x[m].y;
     }
     if (!live) return;
     float* dst = I + (size_t)p * nE * (size_t)nroi + r;
@@ -76,11 +87,7 @@ __global__ void __launch_bounds__(SpecCfg<N>::THREADS) k_spectrum(const float2* 
     for (int m = 0; m < E; ++m) {
         int kbin = tid + T * m;
         int e = ((kbin + N / 2) & (N - 1)) - e_lo;      // position on the ascending energy axis
-        if (e >= 0 && e < nE) {
-            const float v = bose[e] * (x[m].x * x[m].x + x[m].y * x[m].y);
-            // Welch chunks after the first add their share (Eq.(2)); a chunk's launches are stream-ordered
-            dst[(size_t)e * nroi] = accumulate ? dst[(size_t)e * nroi] + v : v;
-        }
+        if (e >= 0 && e < nE) dst[(size_t)e * nroi] = bose[e] * acc[m];
     }
 }
 
@@ -101,8 +108,8 @@ struct SpecCfg2 {
 
 template <int N>
 __global__ void __launch_bounds__(SpecCfg2<N>::THREADS) k_spectrum2(const float2* __restrict__ buf, long long nroi,
-                                                                    size_t probe_stride, int accumulate,
-                                                                    const float2* __restrict__ table,
+                                                                    size_t probe_stride, size_t frame_stride, int nchunks,
+                                                                    size_t chunk_stride, const float2* __restrict__ table,
                                                                     const float* __restrict__ window,
                                                                     const float* __restrict__ bose, int e_lo, int nE,
                                                                     float* __restrict__ I) {
@@ -119,37 +126,41 @@ __global__ void __launch_bounds__(SpecCfg2<N>::THREADS) k_spectrum2(const float2
     const long long r = (long long)blockIdx.x * WQ + c;
     const bool live = r < nroi;
     const float2* src = buf + (size_t)p * probe_stride + (live ? r : 0);
-    float2 x[E];
+    float acc[E];                                  // sum over the Welch chunks of |Phi|^2 (Eq.(2)); I is written once
 #pragma unroll
-    for (int m = 0; m < E; ++m) {
-        const int f = tid + T * m;
-        x[m] = live ? src[(size_t)f * nroi] : make_float2(0.f, 0.f);
-    }
-#pragma unroll
-    for (int m = 0; m < E; ++m) {
-        const float w = window[tid + T * m];
-        x[m] = make_float2(x[m].x * w, x[m].y * w);
-    }
-    cp_async_wait_all();
-    __syncthreads();                               // twiddle table complete
+    for (int m = 0; m < E; ++m) acc[m] = 0.f;
     SyncBlock sync;
-    fft2<N, WQ, false, false>(x, tw + tid, ex, tid, c, sync);
+    for (int ch = 0; ch < nchunks; ++ch, src += chunk_stride) {
+        float2 x[E];
+#pragma unroll
+        for (int m = 0; m < E; ++m) {
+            const int f = tid + T * m;
+            x[m] = live ? src[(size_t)f * frame_stride] : make_float2(0.f, 0.f);
+        }
+#pragma unroll
+        for (int m = 0; m < E; ++m) {
+            const float w = window[tid + T * m];
+            x[m] = make_float2(x[m].x * w, x[m].y * w);
+        }
+        if (ch == 0) cp_async_wait_all();
+        __syncthreads();                           // twiddle table complete / previous chunk's exchange read back
+        fft2<N, WQ, false, false>(x, tw + tid, ex, tid, c, sync);
+#pragma unroll
+        for (int m = 0; m < E; ++m) acc[m] += x[m].x * x[m].x + x[m].y * x[m].y;
+    }
     if (!live) return;
     float* dst = I + (size_t)p * nE * (size_t)nroi + r;
 #pragma unroll
     for (int m = 0; m < E; ++m) {
         const int kbin = tid + T * m;
         const int e = ((kbin + N / 2) & (N - 1)) - e_lo;      // position on the ascending energy axis
-        if (e >= 0 && e < nE) {
-            const float v = bose[e] * (x[m].x * x[m].x + x[m].y * x[m].y);
-            dst[(size_t)e * nroi] = accumulate ? dst[(size_t)e * nroi] + v : v;
-        }
+        if (e >= 0 && e < nE) dst[(size_t)e * nroi] = bose[e] * acc[m];
     }
 }
 
 template <int N>
-static int launch_spec2_n(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int64_t nroi, size_t probe_stride, int accumulate,
-                          const float2* table, const float* d_window, const float* d_bose, int e_lo, int nE, float* d_I,
+static int launch_spec2_n(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int64_t nroi, size_t probe_stride, size_t frame_stride,
+                          int nchunks, size_t chunk_stride, const float2* table, const float* d_window, const float* d_bose, int e_lo, int nE, float* d_I,
                           cudaStream_t st) {
     using C = SpecCfg2<N>;
     const size_t smem = C::smem();
@@ -158,8 +169,8 @@ static int launch_spec2_n(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int6
     int64_t gx = (nroi + C::WQ - 1) / C::WQ;
     for (int p0 = 0; p0 < nprobes; p0 += 32768) {
         int np = nprobes - p0 < 32768 ? nprobes - p0 : 32768;
-        kern<<<dim3((unsigned)gx, np), C::THREADS, smem, st>>>(d_buf + (size_t)p0 * probe_stride, (long long)nroi, probe_stride, accumulate,
-                                                              table, d_window, d_bose, e_lo, nE,
+        kern<<<dim3((unsigned)gx, np), C::THREADS, smem, st>>>(d_buf + (size_t)p0 * probe_stride, (long long)nroi, probe_stride, frame_stride,
+                                                              nchunks, chunk_stride, table, d_window, d_bose, e_lo, nE,
                                                               d_I + (size_t)p0 * nE * (size_t)nroi);
         ctx->launches++;
     }
@@ -168,8 +179,8 @@ static int launch_spec2_n(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int6
 }
 
 template <int N>
-static int launch_spec_n(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int64_t nroi, size_t probe_stride, int accumulate,
-                         const float2* roots,
+static int launch_spec_n(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int64_t nroi, size_t probe_stride, size_t frame_stride,
+                         int nchunks, size_t chunk_stride, const float2* roots,
                          const float* d_window, const float* d_bose, int e_lo, int nE, float* d_I, cudaStream_t st) {
     using C = SpecCfg<N>;
     size_t smem = (size_t)2 * exch_elems(N, C::WQ) * sizeof(float2) + (C::TWREG ? 0 : (size_t)N * sizeof(float2));
@@ -178,8 +189,8 @@ static int launch_spec_n(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int64
     int64_t gx = (nroi + C::WQ - 1) / C::WQ;
     for (int p0 = 0; p0 < nprobes; p0 += 32768) {
         int np = nprobes - p0 < 32768 ? nprobes - p0 : 32768;
-        kern<<<dim3((unsigned)gx, np), C::THREADS, smem, st>>>(d_buf + (size_t)p0 * probe_stride, (long long)nroi, probe_stride, accumulate, roots,
-                                                              d_window, d_bose, e_lo, nE,
+        kern<<<dim3((unsigned)gx, np), C::THREADS, smem, st>>>(d_buf + (size_t)p0 * probe_stride, (long long)nroi, probe_stride, frame_stride,
+                                                              nchunks, chunk_stride, roots, d_window, d_bose, e_lo, nE,
                                                               d_I + (size_t)p0 * nE * (size_t)nroi);
         ctx->launches++;
     }
@@ -236,26 +247,26 @@ int launch_detect(tacaw_ctx* ctx, const float* d_I, int nprobes, int nE, int64_t
 }
 
 int launch_spectrum(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int64_t nroi, int nframes, size_t probe_stride,
-                    int accumulate, const float2* d_roots,
+                    size_t frame_stride, int nchunks, size_t chunk_stride, const float2* d_roots,
                     const float* d_window, const float* d_bose, int e_lo, int nE, float* d_I, cudaStream_t st) {
     static const bool two_exchange = [] { const char* e = getenv("TACAW_SPEC_TWO_EXCHANGE"); return e && atoi(e) != 0; }();
     if (two_exchange) {       // comparison switch: the ping-pong plan for the long series too
         switch (nframes) {
-            case 512: return launch_spec_n<512>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
-            case 1024: return launch_spec_n<1024>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
-            case 2048: return launch_spec_n<2048>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+            case 512: return launch_spec_n<512>(ctx, d_buf, nprobes, nroi, probe_stride, frame_stride, nchunks, chunk_stride, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+            case 1024: return launch_spec_n<1024>(ctx, d_buf, nprobes, nroi, probe_stride, frame_stride, nchunks, chunk_stride, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+            case 2048: return launch_spec_n<2048>(ctx, d_buf, nprobes, nroi, probe_stride, frame_stride, nchunks, chunk_stride, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
         }
     }
     switch (nframes) {
-        case 8: return launch_spec_n<8>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
-        case 16: return launch_spec_n<16>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
-        case 32: return launch_spec_n<32>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
-        case 64: return launch_spec_n<64>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
-        case 128: return launch_spec_n<128>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
-        case 256: return launch_spec_n<256>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
-        case 512: return launch_spec2_n<512>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
-        case 1024: return launch_spec2_n<1024>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
-        case 2048: return launch_spec2_n<2048>(ctx, d_buf, nprobes, nroi, probe_stride, accumulate, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+        case 8: return launch_spec_n<8>(ctx, d_buf, nprobes, nroi, probe_stride, frame_stride, nchunks, chunk_stride, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+        case 16: return launch_spec_n<16>(ctx, d_buf, nprobes, nroi, probe_stride, frame_stride, nchunks, chunk_stride, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+        case 32: return launch_spec_n<32>(ctx, d_buf, nprobes, nroi, probe_stride, frame_stride, nchunks, chunk_stride, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+        case 64: return launch_spec_n<64>(ctx, d_buf, nprobes, nroi, probe_stride, frame_stride, nchunks, chunk_stride, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+        case 128: return launch_spec_n<128>(ctx, d_buf, nprobes, nroi, probe_stride, frame_stride, nchunks, chunk_stride, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+        case 256: return launch_spec_n<256>(ctx, d_buf, nprobes, nroi, probe_stride, frame_stride, nchunks, chunk_stride, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+        case 512: return launch_spec2_n<512>(ctx, d_buf, nprobes, nroi, probe_stride, frame_stride, nchunks, chunk_stride, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+        case 1024: return launch_spec2_n<1024>(ctx, d_buf, nprobes, nroi, probe_stride, frame_stride, nchunks, chunk_stride, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
+        case 2048: return launch_spec2_n<2048>(ctx, d_buf, nprobes, nroi, probe_stride, frame_stride, nchunks, chunk_stride, d_roots, d_window, d_bose, e_lo, nE, d_I, st);
     }
     return fail(ctx, TACAW_E_UNSUPPORTED, "nframes must be a power of two in [8, 2048]");
 }

@@ -49,5 +49,26 @@ def test_reference_arm_rank_gating(monkeypatch, capsys):
 
     class A:
         ref_frames, warmup, steps, gpus = 1, 0, 1, 2
-    bench.run_reference(A, None)
+    bench.run_reference(A, None, 1)
     assert capsys.readouterr().out == ""
+
+
+def test_oracle_plan_is_bounded_for_every_config():
+    """The oracle sample of bench.py (cpu_baseline / --impl reference) stays a bounded piece of the same workload: at most 4
+    probes, whole frames for the small configs, one frame of a z-thinned sample with the same lateral cell, grid and atoms per
+    slice for the large ones."""
+    sys.path.insert(0, ROOT)
+    import bench
+    from paper_2607_02236_b200 import workloads as W
+
+    class A:
+        ref_frames = None
+    for cfg in (1, 2, 3, 4, 5):
+        wl = W.make_workload(cfg, nprobes=128 if cfg == 5 else None)
+        wls, nf, cells = bench.oracle_plan(A, wl)
+        assert wls.nprobes <= 4 and nf >= 1 and (wls.nx, wls.ny, wls.lx) == (wl.nx, wl.ny, wl.lx)
+        assert wls.natoms / wls.nslices_total == wl.natoms / wl.nslices_total
+        if cfg <= 2:
+            assert cells is None and wls.nslices_total == wl.nslices_total
+        if cfg == 5:
+            assert cells is not None and wls.nslices_total < wl.nslices_total

@@ -171,14 +171,20 @@ def test_w7_stationary_on_bin_mode_every_chunk_alike(oracle):
 
 # ------------------------------------------------------------------- library host function vs oracle (CPU)
 @pytest.mark.parametrize("kind,par", [("rect", 0.0), ("hann", 0.0), ("tukey", 0.0), ("tukey", 0.1), ("tukey", 1.0),
-                                      ("blackman_harris", 0.0), ("kaiser", 0.0), ("kaiser", 3 * np.pi), ("kaiser", 5 * np.pi)])
+                                      ("blackman_harris", 0.0), ("kaiser", 0.0), ("kaiser", 3 * np.pi), ("kaiser", 5 * np.pi),
+                                      ("dolph_chebyshev", 100.0), ("dolph_chebyshev", 60.0)])
 def test_make_window_host_matches_oracle(oracle, kind, par):
     from paper_2607_02236_b200 import binding, build
     build.build_lib()
+    # Dolph-Chebyshev: the oracle evaluates cos() of angles up to ~2 pi n/2 (1 ulp of the angle ~ 1e-12 at n = 2048), the
+    # library reduces the angle in integers first; both agree with scipy to their own rounding
+    tol = 1e-12 if kind == "dolph_chebyshev" else 2e-13
     for n in (8, 100, 2048):
-        assert np.max(np.abs(binding.make_window(kind, n, par) - oracle.window_table(kind, n, par))) <= 2e-13
+        assert np.max(np.abs(binding.make_window(kind, n, par) - oracle.window_table(kind, n, par))) <= tol
     with pytest.raises(binding.TacawError):
         binding.make_window("tukey", 16, 1.5)
+    with pytest.raises(binding.TacawError):
+        binding.make_window("dolph_chebyshev", 16, -3.0)
 
 
 # ------------------------------------------------------------------------------------------- GPU parity
@@ -208,6 +214,30 @@ def test_spectrum_welch_vs_oracle(oracle, L, nu, kind, par):
             assert rel_l2(got[p], ref[p]) <= 5e-6                        # north_star bar for spectra: 1e-3
         assert np.max(np.abs(got - ref)) <= 1e-3 * np.max(ref)
         tc.close()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("L,nu,skip,stride,kind,par", [(64, 2, 5, 1, "hann", 0.0), (32, 2, 0, 3, "dolph_chebyshev", 100.0),
+                                                     (512, 2, 7, 2, "hann", 0.0), (16, 4, 200, 1, "rect", 0.0)])
+def test_spectrum_welch_skip_init_and_stride_vs_oracle(oracle, L, nu, skip, stride, kind, par):
+    """trajectory_chunks_skip_init (Listing 1 :443) and the snapshot stride (:140) in tacaw_spectrum_welch."""
+    import torch
+    from paper_2607_02236_b200 import binding, build
+    build.build_lib()
+    rng = np.random.default_rng(L + skip + stride)
+    P, Q = 2, 21
+    Ttot = skip + stride * (3 * L + 5)
+    buf = series(rng, P, Ttot, Q)
+    buf[:, :, 1] += 4.0
+    w = binding.make_window(kind, L, par)
+    ref, Eref, nref = oracle.spectrum_welch(buf, L, nu, 5.0, oracle.window_table(kind, L, par), 300.0, skip_init=skip, stride=stride)
+    tc = binding.Tacaw(16, 16, 5.0, 5.0, 0.037, 9e-4, 1)
+    I, E, n = tc.spectrum_welch(torch.from_numpy(buf).to("cuda", torch.complex64), L, nu, 5.0, w, 300.0, skip_init=skip, stride=stride)
+    assert n == nref and n >= 3 and np.array_equal(E, Eref)
+    got = I.cpu().numpy()
+    for p in range(P):
+        assert rel_l2(got[p], ref[p]) <= 5e-6
+    tc.close()
 
 
 @pytest.mark.gpu
