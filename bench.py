@@ -347,12 +347,13 @@ def main():
     nblocks = max(1, min(wl.nframes // fps, args.steps))          # distinct consecutive frame blocks the steps rotate over
     wl_step = W.make_workload(args.config, nprobes=nprobes, nframes=fps)
     shard_workload(wl_step, rank)
-    r = Runner(wl_step, device=local_rank)                        # frames per block from the free-HBM budget (plan_memory)
-    r.alloc_buffer(fps)
-    dev = r.dev
-    # inputs resident in HBM: positions of every frame block and segment
+    dev = torch.device(f"cuda:{local_rank}")
+    # inputs resident in HBM: positions of every frame block and segment (uploaded first, so that the batch plan below is
+    # sized from the HBM that is really left)
     pos_h = [seg.frames(0, nblocks * fps, wl.dt_fs) for seg in wl.segments]
     pos_d = [torch.from_numpy(p).to(dev) for p in pos_h]
+    r = Runner(wl_step, device=local_rank)                        # frames per block from the free-HBM budget (plan_memory)
+    r.alloc_buffer(fps)
     spec_h = [np.ascontiguousarray(s.species, dtype=np.int32) for s in wl.segments]
     R = r.P
     npix = wl.nx * wl.ny
@@ -453,7 +454,7 @@ def main():
 
     # Welch average over half-length chunks (nu = 2) of the resident time-ordered buffer
     welch = None
-    if fps >= 16:
+    if 16 <= fps <= 512:
         Lc = 1 << ((fps // 2).bit_length() - 1)
         r.spectrum_welch(Lc, 2)
         w0, w1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)

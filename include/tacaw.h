@@ -180,11 +180,28 @@ int tacaw_accumulate(tacaw_ctx *ctx, const void *d_qwaves, int nwaves, const int
                      const int32_t *wave_frame, const int32_t *d_roi_idx, int64_t nroi, void *d_buf,
                      int nprobes, int nframes, void *stream);
 
+/* a5 + a6 fused ("tacaw_propagate + tacaw_accumulate may be fused internally"): the
+ * same multislice run as tacaw_propagate with output_space = 1, but the LAST column kernel writes phi = Psi_S/sqrt(nx ny)
+ * of the ROI pixels straight into buf[wave_probe[w]][wave_time[w]][r] -- the q-space exit wave is neither stored nor
+ * re-read.  Results equal tacaw_propagate + tacaw_accumulate to fp32 rounding (one scale factor instead of two).
+ * d_waves     DEVICE complex64 [nwaves][ny][nx]: scratch for the waves in flight (its content afterwards is unspecified).
+ * wave_probe  HOST int32 [nwaves]: probe of each wave, in [0, nprobes_buf) (also the index into d_probes when non-NULL).
+ * wave_time   HOST int32 [nwaves]: frame index of each wave on the time axis of d_buf, in [0, nframes_buf).
+ * d_roi_inv   DEVICE int32 [ny][nx] from tacaw_make_roi_inverse: position r of a pixel in the ROI list, -1 outside.
+ * Other arguments as tacaw_propagate / tacaw_accumulate. */
+int tacaw_make_roi_inverse(tacaw_ctx *ctx, const int32_t *d_roi_idx, int64_t nroi, int32_t *d_roi_inv, void *stream);
+int tacaw_propagate_accumulate(tacaw_ctx *ctx, void *d_waves, const void *d_probes, int nprobes, const int32_t *wave_probe,
+                               const int32_t *wave_frame, const int32_t *wave_time, int nwaves, const void *const *d_trans,
+                               int nframes_in_flight, const int32_t *nslices_per_segment, int nsegments,
+                               double slice_thickness_A, const int32_t *d_roi_inv, int64_t nroi, void *d_buf,
+                               int nprobes_buf, int nframes_buf, void *stream);
+
 /* O9-O10 spectrum (Eq.(1) :37; :122, :142):
  *   Phi_k = sum_f w_f buf[p][f][r] exp(-2 pi i k f/T);  E_k = h k'/(T dt), k' = k or k-T
  *   I[p][e][r] = B(E_e/(k_B T_K)) |Phi|^2 / (T sum_f w_f^2),  B(x) = x/(1-exp(-x)), B(0) = 1
  * Energies ascending, restricted to [emin_meV, emax_meV] (inclusive, 1e-9 meV slack).
- * nframes: power of two in [8, 2048].
+ * nframes: a power of two in [8, 2048] (register / shared-memory FFT), or any other length in [2, 512] (plain DFT over the
+ * wanted energy bins -- the paper's default chunk of 200 snapshots, :164, gives its 1.4 meV sampling).
  * Series of 512 frames and more run on the single-exchange transform of the slice-step kernels; the environment variable
  * TACAW_SPEC_TWO_EXCHANGE=1 (read once) keeps the two-exchange plan of the shorter series for comparison -- same results.
  * d_I HOST-NULLABLE: pass d_I = NULL to query nE / the axis only.
@@ -205,7 +222,7 @@ int tacaw_make_window(int kind, int n, double param, double *w_out);
  * (:138, remainder-less division, counted in the chunk's own snapshots; reading G24), for every n whose last frame
  * exists (N complete chunks):
  *   I[p][e][r] = (1/N) sum_n B(E_e/(k_B T_K)) |Phi_n|^2 / (L sum_f w_f^2),  Phi_n = DFT over the chunk of w_f buf
- * with E_k = h k'/(L dt frame_stride).  L = chunk_len: power of two in [8, 2048]; nu = chunk_overlap >= 1;
+ * with E_k = h k'/(L dt frame_stride).  L = chunk_len: as nframes of tacaw_spectrum; nu = chunk_overlap >= 1;
  * skip_init >= 0; frame_stride >= 1.  All chunks run in ONE launch (|Phi_n|^2 summed in registers, I written once).
  * window_table HOST double [L] (tacaw_make_window or the caller's own).  N = 0 (buffer shorter than a chunk)
  * leaves d_I untouched.  nchunks HOST out (may be NULL).  Other arguments as tacaw_spectrum;

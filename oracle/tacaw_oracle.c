@@ -222,7 +222,14 @@ int oracle_build_slices(int nx, int ny, double lx, double ly, const double *pos,
         }
     }
     double worst_ratio = 0.0;
-#pragma omp parallel for schedule(dynamic, 1) reduction(max : worst_ratio)
+    /* slices are independent: one thread per slice when there are enough of them; otherwise the slices run one after the
+     * other and the rows of each atom's contribution are shared out instead (every pixel still adds its atoms in the same
+     * order, so the sums are unchanged) */
+    int over_slices = 1;
+#ifdef _OPENMP
+    over_slices = nslices >= omp_get_max_threads();
+#endif
+#pragma omp parallel for schedule(dynamic, 1) reduction(max : worst_ratio) if (over_slices)
     for (int n = 0; n < nslices; ++n) {
         double *V = (double *)calloc(2 * npix, sizeof(double));
         double *ex = (double *)malloc(sizeof(double) * 2 * (size_t)nx);
@@ -241,6 +248,7 @@ int oracle_build_slices(int nx, int ny, double lx, double ly, const double *pos,
                     ey[2 * iy] = cos(ang); ey[2 * iy + 1] = sin(ang);
                 }
             }
+#pragma omp parallel for schedule(static) if (!over_slices)
             for (int iy = 0; iy < ny; ++iy) {
                 int k = signed_index(iy, ny);
                 for (int ix = 0; ix < nx; ++ix) {

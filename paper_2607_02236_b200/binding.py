@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libtacaw.so")
 EXPORTS = ["tacaw_version", "tacaw_create", "tacaw_destroy", "tacaw_last_error", "tacaw_launch_count",
            "tacaw_workspace_bytes", "tacaw_set_workspace", "tacaw_device_status",
            "tacaw_build_slices", "tacaw_build_slices_host", "tacaw_make_probes", "tacaw_propagate",
-           "tacaw_make_roi", "tacaw_accumulate", "tacaw_spectrum", "tacaw_make_window", "tacaw_spectrum_welch",
+           "tacaw_make_roi", "tacaw_accumulate", "tacaw_make_roi_inverse", "tacaw_propagate_accumulate", "tacaw_spectrum", "tacaw_make_window", "tacaw_spectrum_welch",
            "tacaw_make_detector", "tacaw_detect", "tacaw_make_scan", "tacaw_scan_batch"]
 
 DETECTORS = {"circular": 0, "annular": 1}
@@ -271,6 +271,50 @@ class Tacaw:
                                       self._stream())
         self._check(rc, "tacaw_propagate")
         return waves
+
+    def _trans_table(self, trans):
+        torch = self.torch
+        nframes, nseg = len(trans), len(trans[0])
+        ptrs = (C.c_void_p * (nframes * nseg))()
+        nsl = np.array([int(t.shape[0]) for t in trans[0]], dtype=np.int32)
+        for f in range(nframes):
+            if len(trans[f]) != nseg:
+                raise TacawError("every frame needs the same number of segments")
+            for k in range(nseg):
+                t = trans[f][k]
+                if tuple(t.shape) != (int(nsl[k]), self.ny, self.nx):
+                    raise TacawError("transmission tensor has the wrong shape")
+                ptrs[f * nseg + k] = self._dev(t, torch.complex64, "trans").value
+        return ptrs, nsl, nframes, nseg
+
+    def make_roi_inverse(self, roi_idx, out=None):
+        """tacaw_make_roi_inverse: CUDA int32 [ny][nx], position of each pixel in the ROI list or -1."""
+        torch = self.torch
+        if out is None:
+            out = torch.empty((self.ny, self.nx), dtype=torch.int32, device=roi_idx.device)
+        rc = self.lib.tacaw_make_roi_inverse(self._ctx, self._dev(roi_idx, torch.int32, "roi_idx"), C.c_int64(roi_idx.numel()),
+                                             self._dev(out, torch.int32, "roi_inv"), self._stream())
+        self._check(rc, "tacaw_make_roi_inverse")
+        return out
+
+    def propagate_accumulate(self, waves, wave_probe, wave_frame, wave_time, trans, dz: float, roi_inv, nroi: int, buf, probes=None):
+        """tacaw_propagate_accumulate: multislice + fused ROI gather into buf (CUDA complex64 [P][T][Q]); `waves` is scratch."""
+        torch = self.torch
+        nw = waves.shape[0]
+        ptrs, nsl, nframes, nseg = self._trans_table(trans)
+        wp, wf, wt = _i32(wave_probe), _i32(wave_frame), _i32(wave_time)
+        if wp.size != nw or wf.size != nw or wt.size != nw:
+            raise TacawError("wave_probe / wave_frame / wave_time length mismatch")
+        self.reserve(nwaves=nw, nframes=nframes, nsegments=nseg)
+        rc = self.lib.tacaw_propagate_accumulate(
+            self._ctx, self._dev(waves, torch.complex64, "waves"),
+            self._dev(probes, torch.complex64, "probes") if probes is not None else None,
+            C.c_int(int(probes.shape[0]) if probes is not None else 0), wp.ctypes.data_as(C.c_void_p),
+            wf.ctypes.data_as(C.c_void_p), wt.ctypes.data_as(C.c_void_p), C.c_int(nw), ptrs, C.c_int(nframes),
+            nsl.ctypes.data_as(C.c_void_p), C.c_int(nseg), C.c_double(dz), self._dev(roi_inv, torch.int32, "roi_inv"),
+            C.c_int64(nroi), self._dev(buf, torch.complex64, "buf"), C.c_int(buf.shape[0]), C.c_int(buf.shape[1]), self._stream())
+        self._check(rc, "tacaw_propagate_accumulate")
+        return buf
 
     def accumulate(self, qwaves, wave_probe, wave_frame, roi_idx, buf):
         """tacaw_accumulate: buf (CUDA complex64 [P][T][Q]) updated in place."""

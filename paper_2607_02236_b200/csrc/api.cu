@@ -43,7 +43,7 @@ static void region_sizes(const tacaw_ctx* ctx, const tacaw_sizes& z, size_t (&by
     bytes[tacaw_ctx::R_PROBE] = up(sizeof(int) * (size_t)ctx->grid.nx + sizeof(uint32_t) * 2 * nprobes + 64);
     // propagate: wave_frame | wave_probe | tuples (<= (nwaves + 64) * rpt) | transmission pointers
     const size_t rpt = (size_t)row_tuple_size(ctx->grid.nx);
-    bytes[tacaw_ctx::R_PROP] = up(sizeof(int) * (2 * nwaves + (nwaves + 64) * rpt) + 16 + sizeof(void*) * nframes * nseg + 64);
+    bytes[tacaw_ctx::R_PROP] = up(sizeof(int) * (3 * nwaves + (nwaves + 64) * rpt) + 16 + sizeof(void*) * nframes * nseg + 64);
     bytes[tacaw_ctx::R_ACC] = up(sizeof(int) * 2 * nwaves + 64);
     bytes[tacaw_ctx::R_SPEC] = up(SPEC_TABLE_BYTES);
 }
@@ -401,10 +401,19 @@ int tacaw_make_probes(tacaw_ctx* ctx, const double* probe_xy_A, int nprobes, dou
     return TACAW_OK;
 }
 
-int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, int nprobes, const int32_t* wave_probe,
-                    const int32_t* wave_frame, int nwaves, const void* const* d_trans, int nframes,
-                    const int32_t* nslices_per_segment, int nsegments, double dz, int output_space, void* stream) {
-    TACAW_ENTER(ctx);
+// fused gather (a6) of tacaw_propagate_accumulate: where the last column kernel puts the ROI pixels
+struct GatherTarget {
+    const int32_t* wave_time;      // HOST [nwaves] frame index on the buffer's time axis
+    const int* d_roi_inv;          // DEVICE [ny][nx]
+    int64_t nroi;
+    float2* d_buf;
+    int nprobes_buf, nframes_buf;
+};
+
+static int propagate_impl(tacaw_ctx* ctx, void* d_waves, const void* d_probes, int nprobes, const int32_t* wave_probe,
+                          const int32_t* wave_frame, int nwaves, const void* const* d_trans, int nframes,
+                          const int32_t* nslices_per_segment, int nsegments, double dz, int output_space, const GatherTarget* gt,
+                          void* stream) {
     if (nwaves < 0 || nframes <= 0 || nsegments <= 0 || !(dz > 0) || !d_trans || !nslices_per_segment ||
         (nwaves > 0 && (!d_waves || !wave_frame)) || (d_probes && (!wave_probe || nprobes <= 0)) ||
         (output_space != 0 && output_space != 1))
@@ -427,11 +436,11 @@ int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, int npr
     if (rc) return rc;
     const tacaw_grid& g = ctx->grid;
     const size_t npix = (size_t)g.nx * g.ny;
-    // metadata: [wave_frame nwaves][wave_probe nwaves][tuples <= nwaves*rpt][trans ptrs nframes*nseg]
+    // metadata: [wave_frame nwaves][wave_probe nwaves][wave_slot nwaves][tuples <= nwaves*rpt][trans ptrs nframes*nseg]
     const int rpt = row_tuple_size(g.nx);
     size_t nb_i = sizeof(int) * (size_t)nwaves;
     size_t nb_t = sizeof(int) * ((size_t)nwaves + 64) * rpt;
-    size_t off_t = 2 * nb_i;
+    size_t off_t = 3 * nb_i;
     size_t off_p = ((off_t + nb_t + 15) / 16) * 16;
     size_t need = off_p + sizeof(void*) * (size_t)nframes * nsegments + 64;
     void* meta = nullptr;
@@ -439,11 +448,19 @@ int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, int npr
     if (rc) return rc;
     int* d_wf = (int*)meta;
     int* d_wp = d_wf + nwaves;
+    int* d_ws = d_wp + nwaves;
     int* d_tup = (int*)((char*)meta + off_t);
     const float2** d_tp = (const float2**)((char*)meta + off_p);
     if ((rc = upload(ctx, d_wf, wave_frame, nb_i, st))) return rc;
     if (d_probes && (rc = upload(ctx, d_wp, wave_probe, nb_i, st))) return rc;
     if ((rc = upload(ctx, (void*)d_tp, d_trans, sizeof(void*) * (size_t)nframes * nsegments, st))) return rc;
+    if (gt) {
+        std::vector<int> slot(nwaves);
+        for (int w = 0; w < nwaves; ++w) slot[w] = wave_probe[w] * gt->nframes_buf + gt->wave_time[w];
+        if ((rc = upload(ctx, d_ws, slot.data(), nb_i, st))) return rc;
+        // ROI pixels outside the band limit are exactly zero and no column launch reaches them
+        if ((rc = launch_zero_slots(ctx, gt->d_buf, d_ws, nwaves, gt->nroi, st))) return rc;
+    }
 
     // depth-first over groups of waves small enough to stay L2-resident between the two kernels of
     // a slice step: all slices for group 0, then group 1, ...
@@ -525,15 +542,18 @@ int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, int npr
                 ra.pdl = step > 0;      // step 0 may directly follow the kernels that wrote t_n
                 rc = launch_row(ctx, step == 0 ? ROW_FIRST : ROW_MID, ra, st);
                 if (rc) return rc;
-                bool lastq = (step == total - 1) && output_space == 1;
+                const bool lastq = (step == total - 1) && output_space == 1;
+                const bool fused = lastq && gt != nullptr;
                 ColArgs ca{};
                 ca.waves = ra.waves; ca.nwaves = nw; ca.nx = g.nx; ca.hmax = ctx->hmax; ca.roots = ctx->d_roots_y;
                 ca.stack = (float2*)d_waves; ca.stack_waves = nwaves; ca.wave0 = w0;      // one tensor map for the whole call
                 ca.px = ctx->d_px; ca.py = ctx->d_py; ca.kmax = ctx->d_kmax;
-                ca.pscale = lastq ? (float)((double)g.nx * (double)g.ny) : 1.f;
+                // the tables carry 1/(nx ny): Psi_S unnormalised needs nx ny back; phi = Psi_S/sqrt(nx ny) needs sqrt(nx ny)
+                ca.pscale = fused ? (float)std::sqrt((double)g.nx * (double)g.ny) : (lastq ? (float)((double)g.nx * (double)g.ny) : 1.f);
                 ca.kmaxmax = ctx->kmaxmax;
                 ca.pdl = 1;
-                rc = launch_col(ctx, lastq ? COL_LASTQ : COL_MID, ca, g.ny, st);
+                if (fused) { ca.roi_inv = gt->d_roi_inv; ca.wave_slot = d_ws + w0; ca.gbuf = gt->d_buf; ca.gq = gt->nroi; }
+                rc = launch_col(ctx, fused ? COL_GATHER : (lastq ? COL_LASTQ : COL_MID), ca, g.ny, st);
                 if (rc) return rc;
             }
         }
@@ -553,6 +573,36 @@ int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, int npr
         }
     }
     return TACAW_OK;
+}
+
+int tacaw_propagate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, int nprobes, const int32_t* wave_probe,
+                    const int32_t* wave_frame, int nwaves, const void* const* d_trans, int nframes,
+                    const int32_t* nslices_per_segment, int nsegments, double dz, int output_space, void* stream) {
+    TACAW_ENTER(ctx);
+    return propagate_impl(ctx, d_waves, d_probes, nprobes, wave_probe, wave_frame, nwaves, d_trans, nframes, nslices_per_segment,
+                          nsegments, dz, output_space, nullptr, stream);
+}
+
+int tacaw_make_roi_inverse(tacaw_ctx* ctx, const int32_t* d_roi_idx, int64_t nroi, int32_t* d_roi_inv, void* stream) {
+    TACAW_ENTER(ctx);
+    if (nroi < 0 || !d_roi_inv || (nroi > 0 && !d_roi_idx)) return fail(ctx, TACAW_E_ARG, "tacaw_make_roi_inverse: bad argument");
+    return launch_roi_inverse(ctx, d_roi_idx, nroi, d_roi_inv, (cudaStream_t)stream);
+}
+
+int tacaw_propagate_accumulate(tacaw_ctx* ctx, void* d_waves, const void* d_probes, int nprobes, const int32_t* wave_probe,
+                               const int32_t* wave_frame, const int32_t* wave_time, int nwaves, const void* const* d_trans, int nframes,
+                               const int32_t* nslices_per_segment, int nsegments, double dz, const int32_t* d_roi_inv, int64_t nroi,
+                               void* d_buf, int nprobes_buf, int nframes_buf, void* stream) {
+    TACAW_ENTER(ctx);
+    if (nwaves < 0 || nroi < 0 || nprobes_buf <= 0 || nframes_buf <= 0 || (nwaves > 0 && (!wave_probe || !wave_time || !d_roi_inv || !d_buf)))
+        return fail(ctx, TACAW_E_ARG, "tacaw_propagate_accumulate: bad argument");
+    for (int w = 0; w < nwaves; ++w)
+        if (wave_probe[w] < 0 || wave_probe[w] >= nprobes_buf || wave_time[w] < 0 || wave_time[w] >= nframes_buf)
+            return fail(ctx, TACAW_E_ARG, "tacaw_propagate_accumulate: probe/frame index out of range");
+    if (d_probes && nprobes > nprobes_buf) return fail(ctx, TACAW_E_ARG, "tacaw_propagate_accumulate: more probes than the buffer holds");
+    GatherTarget gt{wave_time, d_roi_inv, nroi, (float2*)d_buf, nprobes_buf, nframes_buf};
+    return propagate_impl(ctx, d_waves, d_probes, nprobes, wave_probe, wave_frame, nwaves, d_trans, nframes, nslices_per_segment,
+                          nsegments, dz, 1, &gt, stream);
 }
 
 // O8 by row spans: for a fixed k every predicate is monotone in |h| (disc, annulus) or in h (rect), so the kept h of a row
@@ -665,11 +715,15 @@ int tacaw_accumulate(tacaw_ctx* ctx, const void* d_qwaves, int nwaves, const int
 static int spectrum_core(tacaw_ctx* ctx, const void* d_buf, int nprobes, int64_t nroi, int nframes_total, int L, int first, int step,
                          int stride, int nchunks, double dt_fs, const double* w, double temperature_K, double emin, double emax,
                          float* d_I, double* E_out, int* nE_out, cudaStream_t st, const char* who) {
-    if (L < 8 || L > 2048 || (L & (L - 1))) return fail(ctx, TACAW_E_UNSUPPORTED, std::string(who) + ": the transform length must be a power of two in [8, 2048]");
+    const bool pow2 = L >= 8 && L <= 2048 && (L & (L - 1)) == 0;
+    if (!pow2 && (L < 2 || L > SPEC_DFT_MAX_L))
+        return fail(ctx, TACAW_E_UNSUPPORTED, std::string(who) + ": the transform length must be a power of two in [8, 2048] or any length in [2, " +
+                                                  std::to_string(SPEC_DFT_MAX_L) + "]");
     const double h_mev_fs = 4135.667696, kb_mev = 8.617333262e-2;
     // ascending axis k' = -L/2 .. L/2-1; keep [emin, emax] with 1e-9 meV slack (reading G11)
     int e_lo = -1, nE = 0;
     std::vector<double> E;
+    // k' = -floor(L/2) .. L - floor(L/2) - 1 (for even L the Nyquist bin is the most negative energy)
     for (int i = 0; i < L; ++i) {
         double e = h_mev_fs * (double)(i - L / 2) / ((double)L * dt_fs);
         if (e < emin - 1e-9 || e > emax + 1e-9) continue;
@@ -681,6 +735,32 @@ static int spectrum_core(tacaw_ctx* ctx, const void* d_buf, int nprobes, int64_t
     if (E_out) for (int i = 0; i < nE; ++i) E_out[i] = E[i];
     if (!d_I || nE == 0 || nprobes == 0 || nroi == 0 || nchunks == 0) return TACAW_OK;
     if (!d_buf) return fail(ctx, TACAW_E_ARG, std::string(who) + ": null buffer");
+    if (!pow2) {
+        // generic length: W[e][f] = w_f exp(-2 pi i k_e f/L) for the wanted bins only, then the per-energy factor
+        double sw2g = 0.0;
+        for (int f = 0; f < L; ++f) sw2g += w[f] * w[f];
+        if (!(sw2g > 0)) return fail(ctx, TACAW_E_ARG, std::string(who) + ": window is identically zero");
+        std::vector<float> tabg(2 * (size_t)nE * L + (size_t)nE);
+        for (int i = 0; i < nE; ++i) {
+            const long long kp = (long long)(e_lo + i) - L / 2;           // signed bin
+            for (int f = 0; f < L; ++f) {
+                const long long m = (((kp * f) % L) + L) % L;
+                const double ang = -2.0 * M_PI * (double)m / (double)L;
+                tabg[2 * ((size_t)i * L + f)] = (float)(w[f] * std::cos(ang));
+                tabg[2 * ((size_t)i * L + f) + 1] = (float)(w[f] * std::sin(ang));
+            }
+            const double x = E[i] / (kb_mev * temperature_K);
+            const double B = (x == 0.0) ? 1.0 : x / (-std::expm1(-x));
+            tabg[2 * (size_t)nE * L + i] = (float)(B / ((double)L * sw2g * (double)nchunks));
+        }
+        void* regg = nullptr;
+        int rcg = region(ctx, tacaw_ctx::R_SPEC, sizeof(float) * tabg.size(), &regg, who);
+        if (rcg) return rcg;
+        if ((rcg = upload(ctx, regg, tabg.data(), sizeof(float) * tabg.size(), st))) return rcg;
+        return launch_spectrum_dft(ctx, (const float2*)d_buf + (size_t)first * (size_t)nroi, nprobes, nroi, L,
+                                   (size_t)nframes_total * (size_t)nroi, (size_t)stride * (size_t)nroi, nchunks, (size_t)step * (size_t)nroi,
+                                   (const float2*)regg, (const float*)regg + 2 * (size_t)nE * L, nE, d_I, st);
+    }
     // table region: roots exp(-2 pi i j/L) (L < 512) or the single-exchange twiddle table of fft2.cuh (L >= 512); window; bose
     static const bool two_exchange = [] { const char* e = getenv("TACAW_SPEC_TWO_EXCHANGE"); return e && atoi(e) != 0; }();
     const bool plan2 = L >= 512 && !two_exchange;
@@ -799,7 +879,6 @@ int tacaw_spectrum(tacaw_ctx* ctx, const void* d_buf, int nprobes, int64_t nroi,
     if (nprobes < 0 || nroi < 0 || nframes <= 0 || !(dt_fs > 0) || !(temperature_K > 0) || !nE_out ||
         (window != TACAW_WINDOW_RECT && window != TACAW_WINDOW_HANN))
         return fail(ctx, TACAW_E_ARG, "tacaw_spectrum: bad argument");
-    if (nframes < 8 || nframes > 2048 || (nframes & (nframes - 1))) return fail(ctx, TACAW_E_UNSUPPORTED, "nframes must be a power of two in [8, 2048]");
     std::vector<double> w(nframes);
     tacaw_make_window(window, nframes, 0.0, w.data());
     return spectrum_core(ctx, d_buf, nprobes, nroi, nframes, nframes, 0, nframes, 1, 1, dt_fs, w.data(), temperature_K, emin, emax, d_I,

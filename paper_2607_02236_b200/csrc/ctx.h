@@ -104,7 +104,7 @@ struct AbTable {
 
 // launchers implemented in the kernel translation units --------------------------------------
 enum RowMode { ROW_FIRST = 0, ROW_MID = 1, ROW_LAST = 2, ROW_TRANS = 3 };
-enum ColMode { COL_MID = 0, COL_LASTQ = 1, COL_INV = 2 };
+enum ColMode { COL_MID = 0, COL_LASTQ = 1, COL_INV = 2, COL_GATHER = 3 };
 
 struct RowArgs {
     float2* waves;                 // [nwaves][ny][nx]
@@ -139,6 +139,11 @@ struct ColArgs {
     float pscale;                  // multiplies px*py (1 for COL_MID, nx*ny for COL_LASTQ)
     int pdl;                       // launch as a programmatic dependent of the previous kernel in the stream
     int kmaxmax;                   // largest kmax[ix] of the masked modes (-1: not applicable)
+    // COL_GATHER (fused a6): the ROI pixels of Psi_S go straight into the time-ordered buffer
+    const int* roi_inv;            // device [ny][nx]: ROI position r of a pixel, -1 outside the ROI
+    const int* wave_slot;          // device [nwaves]: probe * nframes_buf + frame of each wave of this launch
+    float2* gbuf;                  // buffer [nprobes][nframes][nroi]
+    long long gq;                  // nroi
 };
 
 int launch_row(tacaw_ctx* ctx, int mode, const RowArgs& a, cudaStream_t st);
@@ -155,9 +160,16 @@ int launch_potential(tacaw_ctx* ctx, const double* d_pos, const int32_t* d_speci
 int launch_potential_tc(tacaw_ctx* ctx, const uint32_t* sx, const uint32_t* sy, const int* offsets, int nspecies, const AbTable& ab,
                         int nslices_total, float2* d_V, cudaStream_t st);
 int potential_tc_max_species();
-constexpr size_t SPEC_TABLE_BYTES = 128 * 1024;     // spectrum region: twiddle/window/Bose tables of one call
+// series of a length that is not a power of two (<= SPEC_DFT_MAX_L): plain DFT restricted to the nE wanted bins, W [nE][L]
+int launch_spectrum_dft(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int64_t nroi, int L, size_t probe_stride, size_t frame_stride,
+                        int nchunks, size_t chunk_stride, const float2* d_W, const float* d_bose, int nE, float* d_I, cudaStream_t st);
+constexpr int SPEC_DFT_MAX_L = 512;
+// spectrum region: twiddle/window/Bose tables of one call, or the [nE][L] DFT table of the generic path
+constexpr size_t SPEC_TABLE_BYTES = (size_t)SPEC_DFT_MAX_L * SPEC_DFT_MAX_L * 8 + 16 * 1024;
 int launch_probe_fill(tacaw_ctx* ctx, const uint32_t* d_uxy /*[P][2] fixed-point fractional*/, int nprobes,
                       const int* d_kap /*[nx]*/, float amp, float2* d_waves, cudaStream_t st);
+int launch_roi_inverse(tacaw_ctx* ctx, const int* d_idx, int64_t nroi, int* d_inv, cudaStream_t st);
+int launch_zero_slots(tacaw_ctx* ctx, float2* d_buf, const int* d_slot, int nwaves, int64_t nroi, cudaStream_t st);
 int launch_gather(tacaw_ctx* ctx, const float2* d_q, int nwaves, const int* d_wp, const int* d_wf, const int* d_idx,
                   int64_t nroi, float2* d_buf, int nprobes, int nframes, cudaStream_t st);
 // probe_stride / frame_stride / chunk_stride: elements between consecutive probes' series blocks, consecutive frames of a

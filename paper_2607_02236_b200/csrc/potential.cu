@@ -8,6 +8,7 @@
 // three quadrants follow from the same four real sums (see k_potential).
 // Phases use fixed-point fractional coordinates U = round(u 2^32): (h*U mod 2^32) is exact
 // integer arithmetic, then sincospif -- fp32 h*x/L would lose ~4e-4 rad at |h| ~ 1000.
+#include <algorithm>
 #include <cstdlib>
 
 #include "ctx.h"
@@ -333,6 +334,44 @@ __global__ void k_gather(const float2* __restrict__ q, const int* __restrict__ w
         float2 v = src[idx[r]];
         dst[r] = make_float2(v.x * scale, v.y * scale);
     }
+}
+
+// inverse ROI map for the fused gather: inv[pixel] = position in the ROI list, -1 elsewhere
+__global__ void k_fill_int(int* __restrict__ p, long long n, int v) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) p[i] = v;
+}
+__global__ void k_roi_scatter(const int* __restrict__ idx, long long nroi, int* __restrict__ inv) {
+    for (long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x; r < nroi; r += (long long)gridDim.x * blockDim.x) inv[idx[r]] = (int)r;
+}
+int launch_roi_inverse(tacaw_ctx* ctx, const int* d_idx, int64_t nroi, int* d_inv, cudaStream_t st) {
+    const long long npix = (long long)ctx->grid.nx * ctx->grid.ny;
+    k_fill_int<<<(unsigned)std::min<long long>((npix + 255) / 256, 4096), 256, 0, st>>>(d_inv, npix, -1);
+    ctx->launches++;
+    if (nroi > 0) {
+        k_roi_scatter<<<(unsigned)std::min<long long>((nroi + 255) / 256, 4096), 256, 0, st>>>(d_idx, (long long)nroi, d_inv);
+        ctx->launches++;
+    }
+    TACAW_CUDA(ctx, cudaGetLastError());
+    return TACAW_OK;
+}
+// buffer rows of the waves about to be gathered: ROI pixels in columns outside the band limit are exactly zero and are
+// never touched by the column kernel
+__global__ void k_zero_slots(float2* __restrict__ buf, const int* __restrict__ slot, long long nroi) {
+    float2* dst = buf + (size_t)slot[blockIdx.y] * (size_t)nroi;
+    for (long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x; r < nroi; r += (long long)gridDim.x * blockDim.x)
+        dst[r] = make_float2(0.f, 0.f);
+}
+int launch_zero_slots(tacaw_ctx* ctx, float2* d_buf, const int* d_slot, int nwaves, int64_t nroi, cudaStream_t st) {
+    if (nwaves <= 0 || nroi <= 0) return TACAW_OK;
+    int bx = (int)((nroi + 255) / 256);
+    if (bx > 64) bx = 64;
+    for (int w0 = 0; w0 < nwaves; w0 += 32768) {
+        const int nw = nwaves - w0 < 32768 ? nwaves - w0 : 32768;
+        k_zero_slots<<<dim3(bx, nw), 256, 0, st>>>(d_buf, d_slot + w0, (long long)nroi);
+        ctx->launches++;
+    }
+    TACAW_CUDA(ctx, cudaGetLastError());
+    return TACAW_OK;
 }
 
 int launch_gather(tacaw_ctx* ctx, const float2* d_q, int nwaves, const int* d_wp, const int* d_wf, const int* d_idx,

@@ -73,9 +73,13 @@ __device__ __forceinline__ float2 phase_fx(uint32_t u, int h) {      // exp(-2 p
 }
 __device__ __forceinline__ float tf32_hi(float x) { return __uint_as_float(__float_as_uint(x) & 0xFFFFE000u); }
 
+constexpr int TC_ATOMS_SMEM = 2048; // sorted coordinates of a species staged per pass (16 KB)
+
 struct TcSmem {
-    float2 coarse[2][2][8][TC_KB];     // [stage][axis][tile row / 8][atom]: exp(-2 pi i (x0 + 8 c) u)
-    float2 fine[2][2][8][TC_KB];       //                 [tile row % 8]     exp(-2 pi i f u)
+    // rows padded to 17 entries (136 B): the 8 rows a quarter-warp reads start in different banks
+    float2 coarse[2][2][8][TC_KB + 1]; // [stage][axis][tile row / 8][atom]: exp(-2 pi i (x0 + 8 c) u)
+    float2 fine[2][2][8][TC_KB + 1];   //                 [tile row % 8]     exp(-2 pi i f u)
+    uint32_t ux[TC_ATOMS_SMEM], uy[TC_ATOMS_SMEM];   // fixed-point coordinates of the species being accumulated
     float gk[TC_MAX_SPECIES][4][TC_TILE];   // exp(-b_sg k^2/ly^2) for the tile's k
     unsigned long long bar_stage[2];   // MMAs that read a stage have completed
     unsigned long long bar_done;       // all MMAs of the tile have completed
@@ -134,6 +138,14 @@ __global__ void __launch_bounds__(TC_THREADS) k_potential_tc(const uint32_t* __r
         for (int base = a0; base < a1; base += TC_KB, ++it) {
             const int st = it & 1;
             const int cnt = min(TC_KB, a1 - base);
+            // coordinates: one coalesced pass per TC_ATOMS_SMEM atoms instead of a dependent global load per k-block
+            const int rel = (base - a0) % TC_ATOMS_SMEM;
+            if (rel == 0) {
+                __syncthreads();                 // the previous pass's coordinates are no longer being read
+                const int nload = min(TC_ATOMS_SMEM, a1 - base);
+                for (int i = lt; i < nload; i += TC_THREADS) { sm.ux[i] = sx[base + i]; sm.uy[i] = sy[base + i]; }
+                __syncthreads();
+            }
             if (it >= 2) {                   // the MMAs that read this stage two k-blocks ago must be done
                 bar_wait(&sm.bar_stage[st], ph[st]);
                 ph[st] ^= 1;
@@ -144,7 +156,7 @@ __global__ void __launch_bounds__(TC_THREADS) k_potential_tc(const uint32_t* __r
                 const int axis = e >> 4, j = e & 15;
                 float2 v = make_float2(0.f, 0.f);               // atoms past the end of the species contribute nothing
                 if (at < cnt) {
-                    const uint32_t u = axis ? sy[base + at] : sx[base + at];
+                    const uint32_t u = axis ? sm.uy[rel + at] : sm.ux[rel + at];
                     v = (j < 8) ? phase_fx(u, (axis ? k0 : h0) + 8 * j) : phase_fx(u, j - 8);
                 }
                 if (j < 8) sm.coarse[st][axis][j][at] = v; else sm.fine[st][axis][j - 8][at] = (at < cnt) ? v : make_float2(0.f, 0.f);

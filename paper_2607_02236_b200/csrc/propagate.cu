@@ -581,7 +581,7 @@ __global__ void __launch_bounds__(ColCfg<N, MODE>::THREADS, ColCfg<N, MODE>::MIN
 #pragma unroll
                 for (int m = 0; m < E; ++m) wmid[(size_t)xt.mid_off(m) * a.nx] = x[m];
             } else {
-                if constexpr (MODE == COL_LASTQ) xt.template first<false, false>(x, ex, sync, hook);
+                if constexpr (MODE == COL_LASTQ || MODE == COL_GATHER) xt.template first<false, false>(x, ex, sync, hook);
                 else xt.template first<false, false>(x, ex, sync, nohook);
 #pragma unroll
                 for (int m = 0; m < E; ++m) {
@@ -596,6 +596,16 @@ __global__ void __launch_bounds__(ColCfg<N, MODE>::THREADS, ColCfg<N, MODE>::MIN
                     xt.template second<true, true>(x, ex, sync, hook);
 #pragma unroll
                     for (int m = 0; m < E; ++m) wc[m * rs] = x[m];
+                } else if constexpr (MODE == COL_GATHER) {
+                    // fused a6: phi = Psi_S / sqrt(nx ny) of the ROI pixels of this column, straight into buf[p][f][r]
+                    const int ixg = group_of(gi) * WC + c;
+                    const int* invc = a.roi_inv + ixg + (size_t)xt.mid0 * a.nx;
+                    float2* gdst = a.gbuf + (size_t)a.wave_slot[w] * (size_t)a.gq;
+#pragma unroll
+                    for (int m = 0; m < E; ++m) {
+                        const int rr = invc[(size_t)xt.mid_off(m) * a.nx];
+                        if (rr >= 0) gdst[rr] = x[m];
+                    }
                 } else {
 #pragma unroll
                     for (int m = 0; m < E; ++m) wmid[(size_t)xt.mid_off(m) * a.nx] = x[m];
@@ -704,6 +714,7 @@ static int launch_col_mode(tacaw_ctx* ctx, int mode, const ColArgs& a, cudaStrea
         case COL_MID: return band ? launch_col_nb<N, COL_MID, true>(ctx, a, st) : launch_col_nb<N, COL_MID, false>(ctx, a, st);
         case COL_LASTQ: return band ? launch_col_nb<N, COL_LASTQ, true>(ctx, a, st) : launch_col_nb<N, COL_LASTQ, false>(ctx, a, st);
         case COL_INV: return launch_col_nb<N, COL_INV, false>(ctx, a, st);
+        case COL_GATHER: return band ? launch_col_nb<N, COL_GATHER, true>(ctx, a, st) : launch_col_nb<N, COL_GATHER, false>(ctx, a, st);
     }
     return fail(ctx, TACAW_E_ARG, "bad column mode");
 }

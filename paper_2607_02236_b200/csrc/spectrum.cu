@@ -198,6 +198,81 @@ static int launch_spec_n(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int64
     return TACAW_OK;
 }
 
+// Series of any other length (the paper's default chunk of 200 snapshots, Listing 1 :442): the time transform as
+// the plain DFT sum restricted to the energy ROI,  Phi_e = sum_f W[e][f] x[f],  W[e][f] = w_f exp(-2 pi i k_e f/L) (host table,
+// fp64 with the phase index k_e f mod L reduced exactly).  A CTA holds a [L x 32 series] tile in shared memory; a warp owns
+// every fourth group of four energies and keeps their four sums in registers, one series per lane (coalesced loads of the
+// buffer, broadcast reads of W).  Work is nE L complex multiply-adds per series -- the spectrum is a small share of the path
+// and with an energy ROI only the wanted bins are computed.
+constexpr int DFT_SER = 32;        // series per CTA
+constexpr int DFT_WARPS = 4;
+constexpr int DFT_EB = 4;          // energies per register block
+
+__global__ void __launch_bounds__(DFT_SER * DFT_WARPS) k_spectrum_dft(const float2* __restrict__ buf, long long nroi, size_t probe_stride,
+                                                                      size_t frame_stride, int nchunks, size_t chunk_stride, int L,
+                                                                      const float2* __restrict__ W, const float* __restrict__ bose,
+                                                                      int nE, float* __restrict__ I) {
+    extern __shared__ __align__(16) float2 xs[];          // [L][DFT_SER] tile of the chunk, then [nE][DFT_SER] sums of |Phi|^2
+    float* accs = reinterpret_cast<float*>(xs + (size_t)L * DFT_SER);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int p = blockIdx.y;
+    const long long r = (long long)blockIdx.x * DFT_SER + lane;
+    const bool live = r < nroi;
+    const float2* src = buf + (size_t)p * probe_stride + (live ? r : 0);
+    for (int e0 = warp * DFT_EB; e0 < nE; e0 += DFT_WARPS * DFT_EB)
+#pragma unroll
+        for (int j = 0; j < DFT_EB; ++j)
+            if (e0 + j < nE) accs[(e0 + j) * DFT_SER + lane] = 0.f;
+    for (int ch = 0; ch < nchunks; ++ch) {
+        __syncthreads();                                  // previous chunk's tile no longer read
+        for (int f = warp; f < L; f += DFT_WARPS)
+            xs[f * DFT_SER + lane] = live ? src[(size_t)ch * chunk_stride + (size_t)f * frame_stride] : make_float2(0.f, 0.f);
+        __syncthreads();
+        // a warp owns the energy groups e0 = (warp + DFT_WARPS g) DFT_EB: only it touches their sums, no barrier in this loop
+        for (int e0 = warp * DFT_EB; e0 < nE; e0 += DFT_WARPS * DFT_EB) {
+            float2 s[DFT_EB];
+#pragma unroll
+            for (int j = 0; j < DFT_EB; ++j) s[j] = make_float2(0.f, 0.f);
+            for (int f = 0; f < L; ++f) {
+                const float2 x = xs[f * DFT_SER + lane];
+#pragma unroll
+                for (int j = 0; j < DFT_EB; ++j) {
+                    const int e = min(e0 + j, nE - 1);
+                    const float2 w = __ldg(W + (size_t)e * L + f);
+                    s[j].x = fmaf(w.x, x.x, fmaf(-w.y, x.y, s[j].x));
+                    s[j].y = fmaf(w.x, x.y, fmaf(w.y, x.x, s[j].y));
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < DFT_EB; ++j)
+                if (e0 + j < nE) accs[(e0 + j) * DFT_SER + lane] += s[j].x * s[j].x + s[j].y * s[j].y;
+        }
+    }
+    if (!live) return;
+    float* dst = I + (size_t)p * nE * (size_t)nroi + r;
+    // (each warp reads back only the sums it wrote)
+    for (int e0 = warp * DFT_EB; e0 < nE; e0 += DFT_WARPS * DFT_EB)
+#pragma unroll
+        for (int j = 0; j < DFT_EB; ++j)
+            if (e0 + j < nE) dst[(size_t)(e0 + j) * nroi] = bose[e0 + j] * accs[(e0 + j) * DFT_SER + lane];
+}
+
+int launch_spectrum_dft(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int64_t nroi, int L, size_t probe_stride, size_t frame_stride,
+                        int nchunks, size_t chunk_stride, const float2* d_W, const float* d_bose, int nE, float* d_I, cudaStream_t st) {
+    const size_t smem = sizeof(float2) * (size_t)L * DFT_SER + sizeof(float) * (size_t)nE * DFT_SER;
+    TACAW_CUDA(ctx, cudaFuncSetAttribute(k_spectrum_dft, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const int64_t gx = (nroi + DFT_SER - 1) / DFT_SER;
+    for (int p0 = 0; p0 < nprobes; p0 += 32768) {
+        const int np = nprobes - p0 < 32768 ? nprobes - p0 : 32768;
+        k_spectrum_dft<<<dim3((unsigned)gx, np), DFT_SER * DFT_WARPS, smem, st>>>(d_buf + (size_t)p0 * probe_stride, (long long)nroi, probe_stride,
+                                                                                frame_stride, nchunks, chunk_stride, L, d_W, d_bose, nE,
+                                                                                d_I + (size_t)p0 * nE * (size_t)nroi);
+        ctx->launches++;
+    }
+    TACAW_CUDA(ctx, cudaGetLastError());
+    return TACAW_OK;
+}
+
 // DetectorSet reduction: out[d][e][p] = sum_r w[d][r] I[p][e][r].  One warp per (p, e) row of I: float4 loads of the
 // row and of up to 8 weight rows (the weights stay in L2/L1), fp32 partial sums per lane, butterfly reduction.  I is
 // read once for all detectors of the call.

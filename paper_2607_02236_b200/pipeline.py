@@ -64,7 +64,7 @@ class Runner:
     """Holds the device-resident state of one computational batch: context, probes, ROI, buffers."""
 
     def __init__(self, wl, device: int = 0, frames_per_block: Optional[int] = None, probes: Optional[Sequence[int]] = None,
-                 budget_bytes: Optional[float] = None):
+                 budget_bytes: Optional[float] = None, fused_gather: bool = True):
         import torch
         self.torch = torch
         self.wl = wl
@@ -74,6 +74,8 @@ class Runner:
         self.P = len(self.probe_ids)
         self.roi_h = make_roi(wl.nx, wl.ny, wl.lx, wl.ly, wl.lam, wl.roi_mode, [p * 1e-3 for p in wl.roi_params_mrad])
         self.roi = torch.from_numpy(self.roi_h).to(self.dev)
+        self.fused_gather = fused_gather       # run_block: tacaw_propagate_accumulate instead of the unfused pair
+        self.roi_inv = self.tc.make_roi_inverse(self.roi) if fused_gather else None
         self.nseg = len(wl.segments)
         self.nsl = [s.nslices for s in wl.segments]
         if budget_bytes is None:
@@ -135,10 +137,21 @@ class Runner:
     def gather_block(self, nf: int, f0: int, wave_probe, wave_frame):
         self.tc.accumulate(self.waves[: nf * self.P], wave_probe, wave_frame + f0, self.roi, self.buf)
 
+    def propagate_gather_block(self, nf: int, f0: int):
+        """tacaw_propagate_accumulate: the last column kernel writes the ROI pixels into the time-ordered buffer."""
+        nw = nf * self.P
+        wave_frame = np.repeat(np.arange(nf, dtype=np.int32), self.P)
+        wave_probe = np.tile(np.arange(self.P, dtype=np.int32), nf)
+        self.tc.propagate_accumulate(self.waves[:nw], wave_probe, wave_frame, wave_frame + f0, self.trans[:nf], self.wl.dz,
+                                     self.roi_inv, int(self.roi.numel()), self.buf, probes=self.probes)
+
     def run_block(self, pos_d, f0: int, nf: int):
         self.build_block(pos_d, nf)
-        _, wp, wf = self.propagate_block(nf, 1)
-        self.gather_block(nf, f0, wp, wf)
+        if self.fused_gather:
+            self.propagate_gather_block(nf, f0)
+        else:
+            _, wp, wf = self.propagate_block(nf, 1)
+            self.gather_block(nf, f0, wp, wf)
 
     def spectrum(self, out=None):
         wl = self.wl
@@ -213,3 +226,35 @@ def run_scan(wl, scan_shape: Sequence[int], batch_shape: Sequence[int], device: 
     finally:
         if runner is not None:
             runner.close()
+
+
+def run_reassembled(wl, offsets: np.ndarray, chunk_len: int, device: int = 0, probes: Optional[Sequence[int]] = None):
+    """Segment re-assembly per averaging chunk: every z-segment of the stack follows ONE trajectory (segment 0 of
+    the workload); for chunk i, stack position k shows that trajectory from snapshot offsets[i][k] on (offsets drawn by the
+    seeded input generator), so chunk frame f is built from trajectory frames offsets[i][k] + f.  Only the pointer table of
+    tacaw_propagate changes: d_trans[f*nsegments + k] points at the transmissions of snapshot offsets[i][k] + f.
+    Returns the time-ordered buffers [nchunks][P][chunk_len][Q] on the device."""
+    import torch
+    r = Runner(wl, device=device, frames_per_block=1, probes=probes)
+    seg = wl.segments[0]
+    nch, nstack = offsets.shape
+    Q = int(r.roi.numel())
+    out = torch.zeros((nch, r.P, chunk_len, Q), dtype=torch.complex64, device=r.dev)
+    # transmissions of every snapshot any (chunk, frame, position) needs, built once
+    need = sorted({int(offsets[i, k]) + f for i in range(nch) for k in range(nstack) for f in range(chunk_len)})
+    slot = {t: j for j, t in enumerate(need)}
+    pos = torch.from_numpy(np.concatenate([seg.frames(t, t + 1, wl.dt_fs) for t in need])).to(r.dev)
+    trans = torch.empty((len(need), seg.nslices, wl.ny, wl.nx), dtype=torch.complex64, device=r.dev)
+    for j0 in range(0, len(need), 16):
+        j1 = min(len(need), j0 + 16)
+        r.tc.build_slices(pos[j0:j1], r.species_d[0], wl.a, wl.b, wl.dz, seg.nslices, 0.0, out=trans[j0:j1])
+    wp = np.arange(r.P, dtype=np.int32)
+    for i in range(nch):
+        waves = torch.empty((chunk_len * r.P, wl.ny, wl.nx), dtype=torch.complex64, device=r.dev)
+        table = [[trans[slot[int(offsets[i, k]) + f]] for k in range(nstack)] for f in range(chunk_len)]
+        wave_frame = np.repeat(np.arange(chunk_len, dtype=np.int32), r.P)
+        wave_probe = np.tile(wp, chunk_len)
+        r.tc.propagate(waves, wave_frame, table, wl.dz, 1, probes=r.probes, wave_probe=wave_probe)
+        r.tc.accumulate(waves, wave_probe, wave_frame, r.roi, out[i])
+    r.close()
+    return out

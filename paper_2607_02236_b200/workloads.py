@@ -305,3 +305,11 @@ def tiny_workload(n: int = 16, ncell: Tuple[int, int, int] = (1, 1, 2), nframes:
     return Workload("tiny", n, n, ncell[0] * a0, ncell[1] * a0, kv, electron_wavelength_A(kv),
                     interaction_sigma(kv), alpha_mrad, probes, nframes, dt_fs, 300.0, 0.5 * c0, [seg],
                     "full", (), sa, sb)
+
+
+def segment_offsets(seed: int, nchunks: int, nstack: int, ntraj: int, chunk_len: int) -> np.ndarray:
+    """Random start snapshots for re-assembling a stack from one trajectory: offsets[i][k] uniform in
+    [0, ntraj - chunk_len], one per (averaging chunk, stack position).  Input generator only: both implementations take the
+    table as an input."""
+    rng = np.random.default_rng(seed)
+    return rng.integers(0, ntraj - chunk_len + 1, size=(nchunks, nstack)).astype(np.int64)

@@ -158,7 +158,7 @@ def test_error_codes(torch, B):
     with pytest.raises(B.TacawError):
         tc.propagate(w, [0], [[t]], -1.0, 1)                   # bad thickness
     with pytest.raises(B.TacawError):
-        tc.spectrum(torch.zeros((1, 48, 5), dtype=torch.complex64, device="cuda"), 5.0, 1, 300.0)   # T not 2^k
+        tc.spectrum(torch.zeros((1, 1000, 5), dtype=torch.complex64, device="cuda"), 5.0, 1, 300.0)   # neither 2^k nor <= 512
     empty = torch.zeros((0, 64, 64), dtype=torch.complex64, device="cuda")
     tc.propagate(empty, [], [[t]], 1.0, 1)                     # empty batch is a no-op
     tc.close()
@@ -281,6 +281,42 @@ def test_spectrum_vs_oracle(torch, B, oracle, T):
         for p in range(P):
             assert rel_l2(got[p], Iref[p]) <= 5e-6
         assert np.max(np.abs(got - Iref) / (Iref + 1e-3 * Iref.max())) <= 1e-3   # weak bins too
+    tc.close()
+
+
+@pytest.mark.parametrize("T", [5, 48, 200, 500])
+def test_spectrum_generic_length_vs_oracle(torch, B, oracle, T):
+    """Series whose length is not a power of two (the paper's chunks of 200 snapshots): plain DFT path."""
+    rng = np.random.default_rng(T)
+    P, Q = 2, 45                                   # ragged Q: not a multiple of the 32-series tile
+    buf = rng.normal(size=(P, T, Q)) + 1j * rng.normal(size=(P, T, Q))
+    buf[:, :, :4] += 20.0
+    tc = B.Tacaw(16, 16, 5.0, 5.0, 0.037, 9e-4, 1)
+    for window, (emin, emax) in ((1, (-np.inf, np.inf)), (0, (-70.0, 41.0))):
+        Iref, Eref = oracle.spectrum(buf, 5.0, window, 300.0, emin, emax)
+        I, E = tc.spectrum(dev(torch, buf, torch.complex64), 5.0, window, 300.0, emin, emax)
+        assert np.array_equal(E, Eref)
+        got = I.cpu().numpy()
+        assert got.shape == Iref.shape
+        for p in range(P):
+            assert rel_l2(got[p], Iref[p]) <= 2e-5
+    tc.close()
+
+
+def test_welch_with_the_papers_chunk_parameters(torch, B, oracle):
+    """PAPER.md:164-168: chunks of 200 snapshots at 15 fs, nu = 2, Hann, E-ROI +-30 THz -> 1.4 meV sampling and 181 bins;
+    here on 700 snapshots after a skip of 100 (5 chunks)."""
+    rng = np.random.default_rng(200)
+    P, Q, L = 1, 33, 200
+    buf = rng.normal(size=(P, 700, Q)) + 1j * rng.normal(size=(P, 700, Q))
+    buf[:, :, 0] += 10.0
+    e30 = W.H_MEV_FS * 30e12 * 1e-15
+    w = B.make_window("hann", L)
+    ref, Eref, nref = oracle.spectrum_welch(buf, L, 2, 15.0, oracle.window_table("hann", L), 300.0, -e30, e30, skip_init=100)
+    tc = B.Tacaw(16, 16, 5.0, 5.0, 0.037, 9e-4, 1)
+    I, E, n = tc.spectrum_welch(dev(torch, buf, torch.complex64), L, 2, 15.0, w, 300.0, -e30, e30, skip_init=100)
+    assert n == nref == 5 and E.size == 181 and np.array_equal(E, Eref) and round(E[1] - E[0], 1) == 1.4
+    assert rel_l2(I.cpu().numpy()[0], ref[0]) <= 2e-5
     tc.close()
 
 
@@ -465,6 +501,64 @@ def test_propagate_multi_group_multi_stream_vs_oracle(torch, B, oracle, n, nw, n
                            [[t[0].astype(np.complex128)] for t in trans], dz, 1)
     for j, i in enumerate(sample):
         assert rel_l2(got[i], ref[j]) <= 2e-5, i
+    tc.close()
+
+
+@pytest.mark.parametrize("cfg,kw", [(2, dict(nframes=8)), (5, dict(nframes=8, ncz=1, nprobes=3)), (1, dict())])
+def test_fused_gather_equals_propagate_plus_accumulate(torch, B, oracle, cfg, kw):
+    """tacaw_propagate_accumulate (the last column kernel writes the ROI pixels) against the unfused pair on the same inputs:
+    equal to fp32 rounding of one scale factor, untouched buffer slots stay untouched, ROI pixels outside the band limit are
+    exact zeros."""
+    from paper_2607_02236_b200.pipeline import Runner
+    wl = W.make_workload(cfg, **kw)
+    if cfg == 1:
+        wl.roi_mode, wl.roi_params_mrad = "full", ()         # full q: most ROI pixels lie outside the band limit
+    outs = []
+    for fused in (False, True):
+        r = Runner(wl, frames_per_block=3, fused_gather=fused)
+        r.alloc_buffer(wl.nframes + 1)                       # one extra time slot that no wave writes
+        r.buf[:, wl.nframes] = 7.0
+        for f0 in range(0, wl.nframes, r.fpb):
+            nf = min(r.fpb, wl.nframes - f0)
+            r.run_block(r.upload_positions(f0, f0 + nf), f0, nf)
+        outs.append(r.buf.cpu().numpy())
+        roi = r.roi_h
+        r.close()
+    a, b = outs
+    assert np.all(b[:, wl.nframes] == 7.0)
+    for p in range(a.shape[0]):
+        for f in range(wl.nframes):
+            assert rel_l2(b[p, f], a[p, f]) <= 3e-7, (p, f)
+    h = np.where(roi % wl.nx < wl.nx // 2, roi % wl.nx, roi % wl.nx - wl.nx)
+    k = np.where(roi // wl.nx < wl.ny // 2, roi // wl.nx, roi // wl.nx - wl.ny)
+    oob = 9 * (h.astype(np.int64) ** 2 + k.astype(np.int64) ** 2) > wl.nx * wl.nx
+    assert np.all(b[:, :wl.nframes][:, :, oob] == 0)
+
+
+def test_segment_reassembly_per_chunk(torch, B, oracle):
+    """'for each averaging chunk ... construct the stacked supercell from randomly selected segments of that
+    trajectory'.  Three stack positions drawn from one 40-snapshot trajectory for two chunks of 8 frames: the time-ordered
+    buffers of both chunks against the oracle's re-assembled run, and their Welch-averaged spectrum."""
+    from oracle import pipeline as OP
+    from paper_2607_02236_b200.pipeline import run_reassembled
+    wl = W.tiny_workload(n=32, ncell=(2, 2, 1), nframes=40, alpha_mrad=25.0)
+    wl.roi_mode, wl.roi_params_mrad = "disc", (40.0,)
+    off = W.segment_offsets(5, 2, 3, 40, 8)
+    assert off.shape == (2, 3) and off.min() >= 0 and off.max() <= 32 and len(set(off.ravel().tolist())) > 1
+    ref = OP.run_reassembled(wl, off, 8)
+    got = run_reassembled(wl, off, 8).cpu().numpy()
+    assert got.shape == ref.shape
+    for i in range(2):
+        for f in range(8):
+            assert rel_l2(got[i, 0, f], ref[i, 0, f]) <= TOL_WAVE
+    # Eq.(2): the chunk spectra are averaged; here chunk by chunk through tacaw_spectrum on the device
+    tc = B.Tacaw(wl.nx, wl.ny, wl.lx, wl.ly, wl.lam, wl.sigma, 1)
+    acc, accr = 0.0, 0.0
+    for i in range(2):
+        I, E = tc.spectrum(dev(torch, got[i], torch.complex64), wl.dt_fs, 1, wl.temperature_K)
+        Ir, Er = oracle.spectrum(ref[i], wl.dt_fs, 1, wl.temperature_K)
+        acc, accr = acc + I.cpu().numpy() / 2, accr + Ir / 2
+    assert rel_l2(acc[0], accr[0]) <= TOL_SPEC
     tc.close()
 
 

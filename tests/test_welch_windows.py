@@ -252,7 +252,7 @@ def test_spectrum_welch_edge_cases(oracle):
     I, E, n = tc.spectrum_welch(buf, 16, 2, 5.0, w, 300.0)              # shorter than one chunk: nothing to average
     assert n == 0 and E.size == 16 and torch.all(I == 0)
     with pytest.raises(binding.TacawError):
-        tc.spectrum_welch(buf, 12, 2, 5.0, np.ones(12), 300.0)          # not a power of two
+        tc.spectrum_welch(buf, 600, 2, 5.0, np.ones(600), 300.0)        # neither a power of two nor <= 512
     with pytest.raises(binding.TacawError):
         tc.spectrum_welch(buf, 8, 0, 5.0, np.ones(8), 300.0)
     with pytest.raises(binding.TacawError):
