@@ -5,14 +5,14 @@ Default workload (N = 1): the largest single-GPU configuration of BASELINE.json,
 fault, 2048^2 grid, 120 slices), as ONE scan sub-batch of 128 probes (rows 0-3 of the 32x32 raster, `scanning_batch_shape`
 4x32, Listing 1 :428).  One "step" = one pass of the whole hot path over a block of 16 consecutive MD frames of
 that batch:
-  tacaw_build_slices (16 frames x 120 slices) -> tacaw_propagate (128 probes x 16 frames x 120 slices) ->
-  tacaw_accumulate (annular q-ROI) -> tacaw_spectrum (window, time FFT, |.|^2, Bose factor, E-ROI).
+  tacaw_build_slices (16 frames x 120 slices) -> tacaw_propagate_accumulate (128 probes x 16 frames x 120 slices, the
+  annular q-ROI gathered by the last column kernel) -> tacaw_spectrum (window, time FFT, |.|^2, Bose factor, E-ROI).
 Consecutive steps take consecutive frame blocks, so the default 4 timed steps cover 64 consecutive frames.
 `value`  : slice-steps/s of the whole step with the inputs (atom positions of every frame) resident in HBM.
 `e2e`    : the same metric through the C ABI with HOST buffers (positions copied H2D from pinned memory inside the timed
            region through tacaw_build_slices_host, the spectrum I(q,E) copied back D2H).
 `roofline`: the fused slice-step kernel pair (k_row + k_col), algorithmic bytes B_step = 16 N^2 + 8 N^2/R per wave and slice
-            over the CUDA-event time of the tacaw_propagate calls inside the timed region.
+            over the CUDA-event time of the tacaw_propagate_accumulate calls inside the timed region.
 `roofline_by_grid`: the same fraction measured in the same run on short samples of configs[2] (512^2) and configs[3] (1024^2).
 `comparison`: cuFFT plan-many and torch.fft.fft2 slice loops on the same grid (library baselines, not the product).
 `cpu_baseline`: the fp64 oracle, as it stands, on a bounded sample of the same workload.
@@ -350,8 +350,8 @@ def main():
     dev = torch.device(f"cuda:{local_rank}")
     # inputs resident in HBM: positions of every frame block and segment (uploaded first, so that the batch plan below is
     # sized from the HBM that is really left)
-    pos_h = [seg.frames(0, nblocks * fps, wl.dt_fs) for seg in wl.segments]
-    pos_d = [torch.from_numpy(p).to(dev) for p in pos_h]
+    # (generated with the workload recipe on the device: the numpy path needs minutes per thousand frames of a 200 000-atom cell)
+    pos_d = [W.frames_on_device(seg, 0, nblocks * fps, wl.dt_fs, dev) for seg in wl.segments]
     r = Runner(wl_step, device=local_rank)                        # frames per block from the free-HBM budget (plan_memory)
     r.alloc_buffer(fps)
     spec_h = [np.ascontiguousarray(s.species, dtype=np.int32) for s in wl.segments]
@@ -369,11 +369,10 @@ def main():
             if timed:
                 e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 e0.record()
-            _, wp, wf = r.propagate_block(nf, 1)
+            r.propagate_gather_block(nf, f0)          # tacaw_propagate_accumulate: the last column kernel gathers the q-ROI
             if timed:
                 e1.record()
                 prop_events.append((e0, e1, nf * R * wl.nslices_total))
-            r.gather_block(nf, f0, wp, wf)
         return r.spectrum()
 
     def barrier():
@@ -423,19 +422,20 @@ def main():
     e2e = None
     if not args.no_e2e:
         I_host = torch.empty(I.shape, dtype=I.dtype).pin_memory()
-        # the step's inputs live in pinned host memory (numpy views of pinned tensors)
-        pos_pin = [torch.from_numpy(p).pin_memory() for p in pos_h]
+        # the step's inputs live in pinned host memory (numpy views of pinned tensors): the frame blocks the e2e steps use
+        nrep = max(1, min(args.steps, 2 if args.config >= 3 else 3))
+        ne2e = min(nblocks, nrep) * fps
+        pos_pin = [p[:ne2e].cpu().pin_memory() for p in pos_d]
         pos_hp = [t.numpy() for t in pos_pin]
-        h2d = sum(p[:fps].nbytes for p in pos_h) + sum(s.nbytes for s in spec_h) * ((fps + r.fpb - 1) // r.fpb)
+        h2d = sum(p[:fps].numel() * 8 for p in pos_pin) + sum(s.nbytes for s in spec_h) * ((fps + r.fpb - 1) // r.fpb)
         d2h = I_host.numel() * 4
 
         def e2e_step(blk: int):
-            base = (blk % nblocks) * fps
+            base = (blk % min(nblocks, nrep)) * fps
             for f0 in range(0, fps, r.fpb):
                 nf = min(r.fpb, fps - f0)
                 r.build_block_host(pos_hp, base + f0, nf)
-                _, wp, wf = r.propagate_block(nf, 1)
-                r.gather_block(nf, f0, wp, wf)
+                r.propagate_gather_block(nf, f0)
             Ie, _ = r.spectrum()
             I_host.copy_(Ie, non_blocking=True)
             torch.cuda.synchronize()
@@ -443,7 +443,6 @@ def main():
         e2e_step(0)
         barrier()
         t0 = time.perf_counter()
-        nrep = max(1, min(args.steps, 2 if args.config >= 3 else 3))
         for i in range(nrep):
             e2e_step(i)
         barrier()

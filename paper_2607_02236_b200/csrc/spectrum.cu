@@ -106,8 +106,14 @@ struct SpecCfg2 {
     static constexpr size_t smem() { return sizeof(float2) * ((size_t)P::TW_ELEMS + XE); }
 };
 
-template <int N>
-__global__ void __launch_bounds__(SpecCfg2<N>::THREADS) k_spectrum2(const float2* __restrict__ buf, long long nroi,
+// Persistent: a CTA walks (tile, chunk) work items with stride gridDim.x.  The [T][WQ] tile of the NEXT item is requested
+// with 8-byte cp.async copies into the exchange buffer as soon as the exchange of the current item has been read back (the
+// buffer is idle during the second radix pass, |.|^2 and the stores), so the strided global reads of one item overlap the
+// arithmetic of the previous one instead of heading every item (round 1: one tile per CTA, DRAM 23 % busy, every warp
+// waiting on its own 32 loads).
+// WELCH = false (one chunk): no accumulator registers, |Phi|^2 goes straight to the store.
+template <int N, bool WELCH>
+__global__ void __launch_bounds__(SpecCfg2<N>::THREADS, (SpecCfg2<N>::THREADS >= 512 ? 1 : 2)) k_spectrum2(const float2* __restrict__ buf, long long nroi, int nprobes,
                                                                     size_t probe_stride, size_t frame_stride, int nchunks,
                                                                     size_t chunk_stride, const float2* __restrict__ table,
                                                                     const float* __restrict__ window,
@@ -122,56 +128,103 @@ __global__ void __launch_bounds__(SpecCfg2<N>::THREADS) k_spectrum2(const float2
     float2* tw = smem;
     float2* ex = smem + P::TW_ELEMS;
     fft2_load_twiddles<N>(tw, table, lt, C::THREADS);
-    const int p = blockIdx.y;
-    const long long r = (long long)blockIdx.x * WQ + c;
-    const bool live = r < nroi;
-    const float2* src = buf + (size_t)p * probe_stride + (live ? r : 0);
-    float acc[E];                                  // sum over the Welch chunks of |Phi|^2 (Eq.(2)); I is written once
+    const long long ntq = (nroi + WQ - 1) / WQ;
+    const long long ntiles = ntq * nprobes;                    // tile = (probe, q tile); a CTA takes tiles blockIdx.x + k gridDim.x
+    auto issue = [&](long long tile, int ch) {                 // and runs all chunks of a tile before the next tile
+        const int p = (int)(tile / ntq);
+        const long long r = (tile - (long long)p * ntq) * WQ + c;
+        const float2* src = buf + (size_t)p * probe_stride + (size_t)ch * chunk_stride + r;
+        if (r < nroi) {
 #pragma unroll
-    for (int m = 0; m < E; ++m) acc[m] = 0.f;
+            for (int m = 0; m < E; ++m) cp_async8(ex + (tid + T * m) * WQ + c, src + (size_t)(tid + T * m) * frame_stride);
+        } else {
+#pragma unroll
+            for (int m = 0; m < E; ++m) ex[(tid + T * m) * WQ + c] = make_float2(0.f, 0.f);
+        }
+        cp_async_commit();
+    };
+    long long tile = blockIdx.x;
+    int ch = 0;
+    if (tile < ntiles) issue(tile, 0);
+    float acc[WELCH ? E : 1];                      // sum over the Welch chunks of |Phi|^2 (Eq.(2)); I is written once per tile
     SyncBlock sync;
-    for (int ch = 0; ch < nchunks; ++ch, src += chunk_stride) {
+    while (tile < ntiles) {
+        if constexpr (WELCH) {
+            if (ch == 0) {
+#pragma unroll
+                for (int m = 0; m < E; ++m) acc[m] = 0.f;
+            }
+        }
+        cp_async_wait_all();
+        __syncthreads();                           // tile (and, the first time, the twiddle table) complete
         float2 x[E];
 #pragma unroll
         for (int m = 0; m < E; ++m) {
-            const int f = tid + T * m;
-            x[m] = live ? src[(size_t)f * frame_stride] : make_float2(0.f, 0.f);
+            const float2 v = ex[(tid + T * m) * WQ + c];
+            const float wm = __ldg(window + tid + T * m);       // 4 N bytes, L1-resident
+            x[m] = make_float2(v.x * wm, v.y * wm);
         }
+        __syncthreads();                           // tile consumed: the exchange may overwrite it
+        const bool last_ch = (ch == nchunks - 1);
+        const long long ntile = last_ch ? tile + gridDim.x : tile;
+        const int nch = last_ch ? 0 : ch + 1;
+        auto nopre = []() {};
+        auto post = [&]() {
+            if (ntile < ntiles) {
+                __syncthreads();                   // exchange read back by every thread
+                issue(ntile, nch);
+            }
+        };
+        Hooks<decltype(nopre), decltype(post)> hook{nopre, post};
+        fft2<N, WQ, false, false>(x, tw + tid, ex, tid, c, sync, hook);
+        if constexpr (WELCH) {
 #pragma unroll
-        for (int m = 0; m < E; ++m) {
-            const float w = window[tid + T * m];
-            x[m] = make_float2(x[m].x * w, x[m].y * w);
+            for (int m = 0; m < E; ++m) acc[m] += x[m].x * x[m].x + x[m].y * x[m].y;
         }
-        if (ch == 0) cp_async_wait_all();
-        __syncthreads();                           // twiddle table complete / previous chunk's exchange read back
-        fft2<N, WQ, false, false>(x, tw + tid, ex, tid, c, sync);
+        if (last_ch) {
+            const int p = (int)(tile / ntq);
+            const long long r = (tile - (long long)p * ntq) * WQ + c;
+            if (r < nroi) {
+                float* dst = I + (size_t)p * nE * (size_t)nroi + r;
 #pragma unroll
-        for (int m = 0; m < E; ++m) acc[m] += x[m].x * x[m].x + x[m].y * x[m].y;
+                for (int m = 0; m < E; ++m) {
+                    const int kbin = tid + T * m;
+                    const int e = ((kbin + N / 2) & (N - 1)) - e_lo;      // position on the ascending energy axis
+                    if (e >= 0 && e < nE) dst[(size_t)e * nroi] = bose[e] * (WELCH ? acc[m] : x[m].x * x[m].x + x[m].y * x[m].y);
+                }
+            }
+        }
+        tile = ntile;
+        ch = nch;
     }
-    if (!live) return;
-    float* dst = I + (size_t)p * nE * (size_t)nroi + r;
-#pragma unroll
-    for (int m = 0; m < E; ++m) {
-        const int kbin = tid + T * m;
-        const int e = ((kbin + N / 2) & (N - 1)) - e_lo;      // position on the ascending energy axis
-        if (e >= 0 && e < nE) dst[(size_t)e * nroi] = bose[e] * acc[m];
-    }
+    cp_async_wait_all();
 }
 
 template <int N>
 static int launch_spec2_n(tacaw_ctx* ctx, const float2* d_buf, int nprobes, int64_t nroi, size_t probe_stride, size_t frame_stride,
-                          int nchunks, size_t chunk_stride, const float2* table, const float* d_window, const float* d_bose, int e_lo, int nE, float* d_I,
+                          int nchunks, size_t chunk_stride, const float2* table,
+                          const float* d_window, const float* d_bose, int e_lo, int nE, float* d_I,
                           cudaStream_t st) {
     using C = SpecCfg2<N>;
     const size_t smem = C::smem();
-    auto kern = k_spectrum2<N>;
-    if (smem > 48 * 1024) TACAW_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    int64_t gx = (nroi + C::WQ - 1) / C::WQ;
-    for (int p0 = 0; p0 < nprobes; p0 += 32768) {
-        int np = nprobes - p0 < 32768 ? nprobes - p0 : 32768;
-        kern<<<dim3((unsigned)gx, np), C::THREADS, smem, st>>>(d_buf + (size_t)p0 * probe_stride, (long long)nroi, probe_stride, frame_stride,
-                                                              nchunks, chunk_stride, table, d_window, d_bose, e_lo, nE,
-                                                              d_I + (size_t)p0 * nE * (size_t)nroi);
+    auto kern = nchunks > 1 ? k_spectrum2<N, true> : k_spectrum2<N, false>;
+    const void* key = (const void*)kern;
+    auto itc = ctx->kernel_occ.find(key);
+    if (itc == ctx->kernel_occ.end()) {
+        if (smem > 48 * 1024) TACAW_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int per_sm = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, C::THREADS, smem) != cudaSuccess || per_sm < 1) {
+            (void)cudaGetLastError();
+            per_sm = 1;
+        }
+        itc = ctx->kernel_occ.emplace(key, per_sm).first;
+    }
+    const long long ntiles = ((nroi + C::WQ - 1) / C::WQ) * (long long)nprobes;
+    long long grid = (long long)ctx->num_sms * itc->second;
+    if (grid > ntiles) grid = ntiles;
+    if (grid > 0) {
+        kern<<<(unsigned)grid, C::THREADS, smem, st>>>(d_buf, (long long)nroi, nprobes, probe_stride, frame_stride, nchunks, chunk_stride, table,
+                                                     d_window, d_bose, e_lo, nE, d_I);
         ctx->launches++;
     }
     TACAW_CUDA(ctx, cudaGetLastError());

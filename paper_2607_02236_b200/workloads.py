@@ -130,6 +130,36 @@ class Segment:
         return out
 
 
+def frames_on_device(seg: "Segment", f0: int, f1: int, dt_fs: float, device, chunk: int = 32):
+    """The same positions as Segment.frames, evaluated with torch float64 on `device` in chunks of frames (same formula; the
+    last bit of a cosine may differ from numpy's).  For benchmarks that keep thousands of frames of a 200 000-atom cell resident:
+    the numpy path needs minutes of host time per thousand frames there.  Parity tests use Segment.frames for both sides."""
+    import torch
+    t_all = torch.arange(f0, f1, dtype=torch.float64, device=device) * dt_fs
+    pos0 = torch.from_numpy(seg.pos0).to(device)
+    out = pos0.unsqueeze(0).repeat(f1 - f0, 1, 1)
+    if seg.kind == "static":
+        return out
+    for c0 in range(0, f1 - f0, chunk):
+        t = t_all[c0:c0 + chunk]
+        o = out[c0:c0 + chunk]
+        if seg.kind == "einstein":
+            ph = torch.from_numpy(seg.einstein_phase).to(device)
+            for m in range(len(seg.einstein_energy_meV)):
+                w = 2.0 * np.pi * float(seg.einstein_energy_meV[m]) / H_MEV_FS
+                o += seg.einstein_amp * torch.cos(w * t[:, None, None] + ph[None, :, m, :])
+            continue
+        ms = seg.modes
+        species = torch.from_numpy(seg.species.astype(np.int64)).to(device)
+        for m in range(len(ms.energy_meV)):
+            w = 2.0 * np.pi * float(ms.energy_meV[m]) / H_MEV_FS
+            kap = torch.from_numpy(ms.kappa[m]).to(device)
+            arg = 2.0 * np.pi * (pos0 @ kap)[None, :] - w * t[:, None] + float(ms.phase[m])
+            amp = torch.from_numpy(ms.amp[m]).to(device)[species]
+            o += (amp[None, :] * torch.cos(arg))[:, :, None] * torch.from_numpy(ms.evec[m]).to(device)[None, None, :]
+    return out
+
+
 @dataclass
 class Workload:
     name: str
