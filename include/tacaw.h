@@ -152,9 +152,10 @@ int tacaw_make_probes(tacaw_ctx *ctx, const double *probe_xy_A, int nprobes, dou
  *             d_trans[f*nsegments+k] -> complex64 [nslices_per_segment[k]][ny][nx]
  * output_space 0: r-space psi_S;  1: q-space Psi_S = FFT2(psi_S), unnormalised, native FFT order. */
 /* Tuning knobs of tacaw_propagate, read from the environment (defaults swept on B200):
- *   TACAW_STREAMS=n        wave groups in flight, caller's stream + n-1 internal ones (default 3, 2 for waves above the group
- *                          budget, i.e. 2048^2; max 4; read once)
- *   TACAW_L2_GROUP_MB=x    bytes of full waves per group (default L2/5, whole row tuples, at least 3 waves; 2 waves at 2048^2)
+ *   TACAW_STREAMS=n        wave groups in flight, caller's stream + n-1 internal ones (default 3; 2 from 1024^2 up; max 4;
+ *                          read once)
+ *   TACAW_L2_GROUP_MB=x    bytes of full waves per group (default L2/4.2 in whole row tuples, at least 3 waves; 5 waves at
+ *                          1024^2, 2 waves at 2048^2)
  *   TACAW_GRID_FRAC=f      fraction of the machine-filling grid a slice-step launch uses (default 1; 0.5-1 measured equal)
  *   TACAW_PDL=0            launch the slice-step kernels without programmatic dependent launch
  * They change scheduling only, never results (tests/test_gpu_parity.py::test_propagate_l2_grouping_is_transparent). */

@@ -465,31 +465,39 @@ static int propagate_impl(tacaw_ctx* ctx, void* d_waves, const void* d_probes, i
     // depth-first over groups of waves small enough to stay L2-resident between the two kernels of
     // a slice step: all slices for group 0, then group 1, ...
     // a few groups are in flight at once (one per stream)
-    // L2/5 (25 MB: 48 waves at 256^2, 12 at 512^2, 3 at 1024^2), swept on B200: 512^2 reaches 0.556 of the roofline with
-    // 12 waves per group, 0.54 with 15 (L2/4), 0.53 with 11
-    size_t budget = ctx->l2_bytes ? ctx->l2_bytes / 5 : (size_t)25 << 20;
+    // Defaults swept on B200 (fraction of the roofline; round 2, with the board at its 1 kW power cap the schedules that keep
+    // more in flight lose SM clock): 512^2, 3 streams: 20 MB 0.533, 25 MB 0.552, 29 MB 0.562, 34 MB 0.563, 42 MB 0.535;
+    // 4 streams lower everywhere.  1024^2 (waves per group, 2 / 3 / 4 streams): 3: 0.468 / 0.485 / 0.470, 5: 0.493 / 0.467 /
+    // 0.440, 6: 0.494 / 0.462 / 0.454.  2048^2: see below.
+    size_t budget = ctx->l2_bytes ? (size_t)(ctx->l2_bytes / 4.2) : (size_t)30 << 20;
     int gmin = 3;
+    bool tuned = true;
     if (const char* e = getenv("TACAW_L2_GROUP_MB")) {
         double mb = atof(e);
         if (mb > 0) {
             budget = (size_t)(mb * 1048576.0);
             gmin = 1;
+            tuned = false;
         }
     }
-    int gmax = (int)(budget / (npix * sizeof(float2)));
+    const size_t wave_bytes = npix * sizeof(float2);
+    int gmax = (int)(budget / wave_bytes);
     if (gmax >= 2 * rpt) gmax -= gmax % rpt;      // whole row tuples: a short tuple repeats its last wave (wasted work)
     // A wave larger than the budget (2048^2: 33.6 MB, 22.4 MB in band): what stays L2-resident is the TOTAL in flight, and
     // beyond ~90 MB of in-band waves plus the streaming t_n slice (33.6 MB) the 126 MB L2 thrashes.  Swept on B200 (streams x
     // waves per group, fraction of the roofline): 1x3 0.326, 2x2 0.346, 2x3 0.333, 3x2 0.326, 3x3 0.331, any x4 0.27-0.28.
-    const bool huge = gmax < 2;
-    if (gmax < gmin) gmax = huge ? 2 : gmin;
+    const bool huge = tuned && gmax < 2;
+    const bool large = tuned && !huge && wave_bytes >= ((size_t)8 << 20);      // 1024^2: two streams x five waves
+    if (huge) gmax = 2;
+    else if (large) gmax = 5;
+    else if (gmax < gmin) gmax = gmin;
     const int ngroups = (nwaves + gmax - 1) / gmax;
     static const int env_streams = [] {
         const char* e = getenv("TACAW_STREAMS");
         int v = e ? atoi(e) : 0;
         return v < 0 ? 0 : (v > 1 + tacaw_ctx::MAX_AUX ? 1 + tacaw_ctx::MAX_AUX : v);
     }();
-    const int max_streams = env_streams ? env_streams : (huge ? 2 : 3);
+    const int max_streams = env_streams ? env_streams : ((huge || large) ? 2 : 3);
     const int nstreams = ngroups < max_streams ? ngroups : max_streams;
     const bool fork = nstreams >= 2;
     cudaStream_t user_st = st;
