@@ -285,6 +285,29 @@ int tacaw_build_slices_host(tacaw_ctx *ctx, const double *h_pos_A, const int32_t
                             const tacaw_species *species, double slice_thickness_A, int nslices, double z0_A,
                             void *d_trans, int *n_clamped, void *stream);
 
+/* tacaw_build_slices without a workspace, for callers that cannot allocate device memory (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc).  Same operation, arguments, layouts and result as
+ * tacaw_build_slices (Eq.(1)-(2); O1-O3) minus n_clamped; the scratch of the binning step and
+ * of K1 (clamp counter, keys, fixed-point coordinates, sorted coordinates, per-(frame, slice, species) counts and
+ * offsets) lives in ONE static device array of TACAW_STATIC_SCRATCH_BYTES inside the library instead of the caller's
+ * workspace, so the call works on a context that never had tacaw_set_workspace called.  Every GPU that loads the library
+ * holds those 4 MiB until the process exits.  The call issues no cudaMalloc / cudaFree / allocating library routine and
+ * does not synchronise; it is asynchronous on `stream`.
+ * Limit: 256 + 4*(5*natoms*nframes + 2*nframes*nslices*nspecies + 2) <= TACAW_STATIC_SCRATCH_BYTES (about 200 000
+ *   atom-frames); anything larger returns TACAW_E_UNSUPPORTED before any work is queued (tacaw_last_error states the
+ *   bytes needed and the limit) -- use tacaw_build_slices with a workspace then.
+ * Sharing: every call on a device, from any context, uses the same array, and the array keeps the last call's
+ *   contents.  The counters that must start at zero are cleared on `stream` at the start of each call, so calls
+ *   ordered on one stream (or ordered by events) are independent; two calls that OVERLAP on the GPU (different streams
+ *   without ordering, different contexts or threads on the same device) race on the array and give undefined
+ *   transmissions.  tacaw_build_slices (workspace) and this call do not share scratch.
+ * Out-of-range species ids raise the context's sticky flag exactly as in tacaw_build_slices (tacaw_device_status).
+ * d_pos_A, d_species, d_trans: DEVICE, caller-owned, as in tacaw_build_slices. */
+#define TACAW_STATIC_SCRATCH_BYTES (4u << 20)
+int tacaw_build_slices_static(tacaw_ctx *ctx, const double *d_pos_A, const int32_t *d_species, int natoms, int nframes,
+                              const tacaw_species *species, double slice_thickness_A, int nslices, double z0_A,
+                              void *d_trans, void *stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -19,7 +19,9 @@ EXPORTS = ["tacaw_version", "tacaw_create", "tacaw_destroy", "tacaw_last_error",
            "tacaw_workspace_bytes", "tacaw_set_workspace", "tacaw_device_status",
            "tacaw_build_slices", "tacaw_build_slices_host", "tacaw_make_probes", "tacaw_propagate",
            "tacaw_make_roi", "tacaw_accumulate", "tacaw_make_roi_inverse", "tacaw_propagate_accumulate", "tacaw_spectrum", "tacaw_make_window", "tacaw_spectrum_welch",
-           "tacaw_make_detector", "tacaw_detect", "tacaw_make_scan", "tacaw_scan_batch"]
+           "tacaw_make_detector", "tacaw_detect", "tacaw_make_scan", "tacaw_scan_batch", "tacaw_build_slices_static"]
+
+STATIC_SCRATCH_BYTES = 4 << 20     # TACAW_STATIC_SCRATCH_BYTES of include/tacaw.h
 
 DETECTORS = {"circular": 0, "annular": 1}
 
@@ -207,6 +209,22 @@ class Tacaw:
                                          C.byref(ncl) if want_clamped else None, self._stream())
         self._check(rc, "tacaw_build_slices")
         return out, (int(ncl.value) if want_clamped else None)
+
+    def build_slices_static(self, pos, species, a, b, dz: float, nslices: int, z0: float, out):
+        """tacaw_build_slices_static: same result as build_slices with the scratch in the library's static device array.
+        Allocates nothing (the caller passes `out`) and needs no workspace; sizes beyond STATIC_SCRATCH_BYTES raise."""
+        torch = self.torch
+        nframes = 1 if pos.dim() == 2 else int(pos.shape[0])
+        natoms = int(pos.shape[-2])
+        if out.numel() != nframes * nslices * self.ny * self.nx:
+            raise TacawError("build_slices_static: output tensor has the wrong size")
+        sp, keep = self._species(a, b)
+        rc = self.lib.tacaw_build_slices_static(self._ctx, self._dev(pos, torch.float64, "pos"),
+                                                self._dev(species, torch.int32, "species"), C.c_int(natoms),
+                                                C.c_int(nframes), C.byref(sp), C.c_double(dz), C.c_int(nslices),
+                                                C.c_double(z0), self._dev(out, torch.complex64, "trans"), self._stream())
+        self._check(rc, "tacaw_build_slices_static")
+        return out
 
     def build_slices_host(self, pos_h: np.ndarray, species_h: np.ndarray, a, b, dz: float, nslices: int,
                           z0: float, out, want_clamped: bool = True):

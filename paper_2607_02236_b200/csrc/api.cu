@@ -313,6 +313,38 @@ int tacaw_build_slices(tacaw_ctx* ctx, const double* d_pos_A, const int32_t* d_s
     return TACAW_OK;
 }
 
+int tacaw_build_slices_static(tacaw_ctx* ctx, const double* d_pos_A, const int32_t* d_species, int natoms, int nframes,
+                              const tacaw_species* species, double dz, int nslices, double z0, void* d_trans, void* stream) {
+    TACAW_ENTER(ctx);
+    if (nframes == 0) return TACAW_OK;
+    if (natoms < 0 || nframes < 0 || nslices <= 0 || !(dz > 0) || !d_trans || !species || species->nspecies <= 0 || !species->a ||
+        !species->b || (natoms > 0 && (!d_pos_A || !d_species)))
+        return fail(ctx, TACAW_E_ARG, "tacaw_build_slices_static: bad argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    const int ns = species->nspecies;
+    const int nx = ctx->grid.nx, ny = ctx->grid.ny;
+    if (ns > MAX_SPECIES) return fail(ctx, TACAW_E_UNSUPPORTED, "tacaw_build_slices_static: at most 8 species");
+    AbTable ab{};
+    for (int s = 0; s < ns; ++s)
+        for (int i = 0; i < 4; ++i) {
+            ab.a[s][i] = (float)species->a[4 * s + i];
+            ab.b[s][i] = (float)species->b[4 * s + i];
+        }
+    // sizes beyond the static array are refused before anything is queued
+    int rc = launch_potential_static(ctx, d_pos_A, d_species, natoms, nframes, ns, ab, dz, nslices, z0, (float2*)d_trans, st);
+    if (rc) return rc;
+    // V(q) -> v(r) -> t = exp(i sigma v), as in tacaw_build_slices (these two kernels use no scratch)
+    ColArgs ca{};
+    ca.waves = (float2*)d_trans; ca.nwaves = nframes * nslices; ca.nx = nx; ca.hmax = ctx->hmax_pot; ca.roots = ctx->d_roots_y;
+    ca.px = nullptr; ca.py = nullptr; ca.kmax = ctx->d_kmax_pot; ca.pscale = 1.f; ca.kmaxmax = -1;
+    rc = launch_col(ctx, COL_INV, ca, ny, st);
+    if (rc) return rc;
+    RowArgs ra{};
+    ra.waves = (float2*)d_trans; ra.nwaves = nframes * nslices; ra.ny = ny; ra.hmax = ctx->hmax_pot; ra.roots = ctx->d_roots_x;
+    ra.scale = (float)(ctx->beam.sigma_rad_per_VA / (ctx->grid.lx_A * ctx->grid.ly_A));
+    return launch_row(ctx, ROW_TRANS, ra, st);
+}
+
 int tacaw_build_slices_host(tacaw_ctx* ctx, const double* h_pos_A, const int32_t* h_species, int natoms, int nframes,
                             const tacaw_species* species, double dz, int nslices, double z0, void* d_trans,
                             int* n_clamped, void* stream) {

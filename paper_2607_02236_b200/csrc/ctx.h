@@ -156,6 +156,9 @@ int launch_col(tacaw_ctx* ctx, int mode, const ColArgs& a, int ny, cudaStream_t 
 int launch_potential(tacaw_ctx* ctx, const double* d_pos, const int32_t* d_species, int natoms, int nframes, int nspecies,
                      const AbTable& ab, double dz, int nslices, double z0, float2* d_V, int** d_nclamped,
                      cudaStream_t st);
+// the same with the build region in a static device array of TACAW_STATIC_SCRATCH_BYTES (potential.cu); no workspace needed
+int launch_potential_static(tacaw_ctx* ctx, const double* d_pos, const int32_t* d_species, int natoms, int nframes, int nspecies,
+                            const AbTable& ab, double dz, int nslices, double z0, float2* d_V, cudaStream_t st);
 // tensor-core K1 (potential_tc.cu): sorted fixed-point coordinates and per-(slice, species) offsets -> V(q) of every slice
 int launch_potential_tc(tacaw_ctx* ctx, const uint32_t* sx, const uint32_t* sy, const int* offsets, int nspecies, const AbTable& ab,
                         int nslices_total, float2* d_V, cudaStream_t st);

@@ -10,6 +10,7 @@
 // integer arithmetic, then sincospif -- fp32 h*x/L would lose ~4e-4 rad at |h| ~ 1000.
 #include <algorithm>
 #include <cstdlib>
+#include <mutex>
 
 #include "ctx.h"
 
@@ -275,6 +276,94 @@ int launch_potential(tacaw_ctx* ctx, const double* d_pos, const int32_t* d_speci
         const int total_slices = nframes * nslices;
         // K1 on the tensor cores (potential_tc.cu) unless TACAW_K1_TC=0 asks for the fp32-pipe kernel below (kept for
         // comparison and for more than four species)
+        static const bool use_tc = [] { const char* e = getenv("TACAW_K1_TC"); return e ? atoi(e) != 0 : true; }();
+        if (use_tc && nspecies <= potential_tc_max_species())
+            return launch_potential_tc(ctx, sx, sy, offsets, nspecies, ab, total_slices, d_V, st);
+        for (int z0i = 0; z0i < total_slices; z0i += 65535) {
+            int nz = total_slices - z0i < 65535 ? total_slices - z0i : 65535;
+            dim3 grid((hmax + 1 + POT_T - 1) / POT_T, (ctx->kmaxmax_pot + 1 + POT_T - 1) / POT_T, nz);
+            k_potential<<<grid, POT_THREADS, 0, st>>>(sx, sy, offsets + (size_t)z0i * nspecies, nspecies, ab, ctx->d_kmax_pot, hmax, nx,
+                                              ny, (float)(1.0 / ctx->grid.lx_A), (float)(1.0 / ctx->grid.ly_A),
+                                              d_V + (size_t)z0i * nx * ny);
+            ctx->launches++;
+        }
+    }
+    TACAW_CUDA(ctx, cudaGetLastError());
+    return TACAW_OK;
+}
+
+// ---------------------------------------------------------------------------------------- a1 + K1 without a workspace
+// tacaw_build_slices_static (tacaw.h): the same kernels as launch_potential, with the build region (clamp counter, keys,
+// fixed-point coordinates, sorted coordinates, counts, offsets) in this file-scope device array instead of the caller's
+// workspace, for callers that cannot allocate.  Every GPU that loads the library holds the array until the process exits.
+// All calls on a device share it and it keeps the previous call's contents: the counters are cleared on the caller's
+// stream at the start of every call, and two calls that overlap on the GPU race.
+static __device__ __align__(256) unsigned char g_static_build[TACAW_STATIC_SCRATCH_BYTES];
+
+// In host code `g_static_build` is only a handle for the runtime, not a device address: resolve it once per device, with
+// that device current (TACAW_ENTER in the entry point), and hand the kernels the resolved pointer.
+constexpr int STATIC_MAX_DEVICES = 64;
+static void* g_static_build_ptr[STATIC_MAX_DEVICES];
+static std::mutex g_static_build_mu;
+
+static int static_build_region(tacaw_ctx* ctx, void** out) {
+    if (ctx->device < 0 || ctx->device >= STATIC_MAX_DEVICES)
+        return fail(ctx, TACAW_E_UNSUPPORTED, "tacaw_build_slices_static: device ordinal beyond 63");
+    std::lock_guard<std::mutex> lock(g_static_build_mu);
+    if (!g_static_build_ptr[ctx->device]) {
+        void* p = nullptr;
+        TACAW_CUDA(ctx, cudaGetSymbolAddress(&p, g_static_build));
+        if (!p) return fail(ctx, TACAW_E_CUDA, "tacaw_build_slices_static: cudaGetSymbolAddress returned a null address");
+        g_static_build_ptr[ctx->device] = p;
+    }
+    *out = g_static_build_ptr[ctx->device];
+    return TACAW_OK;
+}
+
+int launch_potential_static(tacaw_ctx* ctx, const double* d_pos, const int32_t* d_species, int natoms, int nframes, int nspecies,
+                            const AbTable& ab, double dz, int nslices, double z0, float2* d_V, cudaStream_t st) {
+    const int nx = ctx->grid.nx, ny = ctx->grid.ny;
+    const long long ntotal = (long long)natoms * nframes;
+    const long long nkeys_ll = (long long)nframes * nslices * nspecies;
+    // same layout as the build region of the workspace: clamp counter (256 B) | keys ux uy sx sy [nt] | counts | offsets
+    const long long nt_ll = ntotal > 0 ? ntotal : 1;
+    const long long need = 256 + (long long)sizeof(int) * (5 * nt_ll + 2 * nkeys_ll + 2);
+    if (ntotal > (1LL << 31) - 1 || nkeys_ll > (1LL << 30) || need > (long long)TACAW_STATIC_SCRATCH_BYTES)
+        return fail(ctx, TACAW_E_UNSUPPORTED,
+                    "tacaw_build_slices_static: this call needs " + std::to_string(need) + " bytes of scratch (256 + 4*(5*natoms*nframes + "
+                    "2*nframes*nslices*nspecies + 2)), the static array holds " + std::to_string((long long)TACAW_STATIC_SCRATCH_BYTES) +
+                    ": use tacaw_build_slices with a workspace");
+    void* reg = nullptr;
+    int rc = static_build_region(ctx, &reg);
+    if (rc) return rc;
+    const int nkeys = (int)nkeys_ll;
+    const size_t nt = (size_t)nt_ll;
+    int* d_nclamped = (int*)reg;
+    int* keys = (int*)((char*)reg + 256);
+    uint32_t* ux = (uint32_t*)(keys + nt);
+    uint32_t* uy = ux + nt;
+    uint32_t* sx = uy + nt;
+    uint32_t* sy = sx + nt;
+    int* counts = (int*)(sy + nt);
+    int* offsets = counts + nkeys;
+    // what must start at zero: the per-key counts (atomicAdd targets), the offsets, the clamp counter
+    TACAW_CUDA(ctx, cudaMemsetAsync(counts, 0, sizeof(int) * (2 * (size_t)nkeys + 1), st));
+    TACAW_CUDA(ctx, cudaMemsetAsync(d_nclamped, 0, sizeof(int), st));
+    if (ntotal == 0) TACAW_CUDA(ctx, cudaMemsetAsync(d_V, 0, sizeof(float2) * (size_t)nframes * nslices * nx * ny, st));
+    if (ntotal > 0) {
+        k_atom_keys<<<(unsigned)((ntotal + 255) / 256), 256, 0, st>>>(d_pos, d_species, natoms, ntotal, nspecies, dz, nslices,
+                                                                     z0, 1.0 / ctx->grid.lx_A, 1.0 / ctx->grid.ly_A, keys, ux,
+                                                                     uy, counts, d_nclamped, ctx->d_flags);
+        ctx->launches++;
+    }
+    k_scan_counts<<<1, 1024, 0, st>>>(counts, nkeys, offsets);
+    ctx->launches++;
+    if (ntotal > 0) {
+        k_compact<<<(unsigned)(((long long)nkeys * 32 + 255) / 256), 256, 0, st>>>(keys, natoms, nslices * nspecies, nkeys, offsets,
+                                                                                  ux, uy, sx, sy);
+        ctx->launches++;
+        const int hmax = ctx->hmax_pot;
+        const int total_slices = nframes * nslices;
         static const bool use_tc = [] { const char* e = getenv("TACAW_K1_TC"); return e ? atoi(e) != 0 : true; }();
         if (use_tc && nspecies <= potential_tc_max_species())
             return launch_potential_tc(ctx, sx, sy, offsets, nspecies, ab, total_slices, d_V, st);
