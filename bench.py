@@ -360,6 +360,7 @@ def main():
     b_step = 16 * npix + 8 * npix / R
     units_per_step = R * fps * wl.nslices_total
     prop_events = []
+    host_issue = [0.0, 0]      # host wall time inside the asynchronous propagate calls, launches they issued
 
     def one_step(blk: int, timed: bool):
         base = (blk % nblocks) * fps
@@ -369,8 +370,11 @@ def main():
             if timed:
                 e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 e0.record()
+                h0, n0 = time.perf_counter(), r.tc.launches
             r.propagate_gather_block(nf, f0)          # tacaw_propagate_accumulate: the last column kernel gathers the q-ROI
             if timed:
+                host_issue[0] += time.perf_counter() - h0
+                host_issue[1] += r.tc.launches - n0
                 e1.record()
                 prop_events.append((e0, e1, nf * R * wl.nslices_total))
         return r.spectrum()
@@ -415,6 +419,12 @@ def main():
                 "fp32 pipe and L1TEX (DESIGN.md section 9)",
                 "peak_source": peak_src, "propagate_share_of_step": prop_ms / elapsed_ms,
                 "propagate_slice_steps_per_s": prop_units / (prop_ms * 1e-3)}
+    if host_issue[1] > 0:
+        # the call returns without synchronising: below ~1000 launches per call (the depth of the driver's launch queue) this is
+        # the host's issue cost per launch; beyond that the host blocks on the queue and the figure tends to the GPU time
+        roofline["host_issue_us_per_launch"] = host_issue[0] * 1e6 / host_issue[1]
+        roofline["gpu_us_per_launch"] = prop_ms * 1e3 / host_issue[1]
+        roofline["launches_per_propagate_call"] = host_issue[1] / max(1, len(prop_events))
     if traffic is not None:
         roofline["dram_frac"] = traffic * (prop_units / (prop_ms * 1e-3)) / 1e9 / peak
 

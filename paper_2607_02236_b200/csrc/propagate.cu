@@ -27,6 +27,12 @@
 #ifndef TACAW_ROW2048_TEAMS
 #define TACAW_ROW2048_TEAMS 2
 #endif
+#ifndef TACAW_ROW2048_MINB
+#define TACAW_ROW2048_MINB 3
+#endif
+#ifndef TACAW_COL2048_REGCAP
+#define TACAW_COL2048_REGCAP 1
+#endif
 #ifndef TACAW_COL2048_MERGE
 #define TACAW_COL2048_MERGE 0
 #endif
@@ -73,7 +79,9 @@ struct RowCfg {
     static constexpr int TEAMS = (N >= 2048) ? TACAW_ROW2048_TEAMS : 4;       // teams per CTA
     static constexpr int THREADS = TEAMS * TEAM;
     static constexpr int XE = X::exch(1);                   // exchange elements per row
-    static constexpr int MINB = (N >= 2048) ? 1 : 3;
+    // three CTAs (12 warps) per SM at every size: at 2048 this caps the pair-plan kernel at 168 registers (it took 174
+    // with the cap at 255), TACAW_ROW2048_MINB=1 restores two CTAs (8 warps) per SM
+    static constexpr int MINB = (N >= 2048) ? TACAW_ROW2048_MINB : 3;
     static constexpr bool CW_SMEM = !X::PAIR || (TACAW_ROW2048_CW_SMEM != 0);
     static constexpr int TW = CW_SMEM ? X::TW_ELEMS : X::P::TW_ELEMS;     // twiddle entries held in shared memory
     // staged t_n row: in the paired ownership a lane pair reads elements 512 apart, i.e. the same banks; every block of 512
@@ -442,6 +450,11 @@ struct ColCfg {
     // 84 KB instead of 148 KB per CTA, so two CTAs (16 warps) fit an SM
     static constexpr bool MERGE = X::PAIR && (TACAW_COL2048_MERGE != 0);
     static constexpr int MINB = (N <= 1024) ? 3 : (MERGE ? 2 : 1);
+    // Register cap through the thread count of __launch_bounds__ (a launch may use fewer threads than it declares): 2048 runs
+    // one 256-thread CTA per SM (shared memory), and ptxas then takes 226 registers because it may.  Declared for 384 threads
+    // the cap is 168 (no spills; 400 threads already round up to 16 warps and a cap of 128, which spills), which leaves room for one row-kernel CTA of the other stream's wave group on the same SM
+    // (256 x 168 + 128 x 168 registers, 149 + 75 KB of shared memory).
+    static constexpr int LB_THREADS = (X::PAIR && !MERGE && TACAW_COL2048_REGCAP) ? 384 : THREADS;
     // twiddles | Py | (pad to 128 B) staging tile [N][WC] (TMA destination) | exchange | mbarrier
     static constexpr int OFF_S = ((X::TW_ELEMS + (PY_SMEM ? N : 0)) + 15) / 16 * 16;
     static constexpr int RB = (N < 256) ? N : 256;            // rows per TMA box
@@ -457,7 +470,7 @@ struct ColCfg {
 // BAND: every kmax[ix] <= N/3, so the chunks of k strictly between N/3 and N - N/3 are masked for
 // every column and are neither multiplied nor tested (single-exchange plans; the pair plan tests every element).
 template <int N, int MODE, bool BAND>
-__global__ void __launch_bounds__(ColCfg<N, MODE>::THREADS, ColCfg<N, MODE>::MINB) k_col(ColArgs a, const __grid_constant__ CUtensorMap tm) {
+__global__ void __launch_bounds__(ColCfg<N, MODE>::LB_THREADS, ColCfg<N, MODE>::MINB) k_col(ColArgs a, const __grid_constant__ CUtensorMap tm) {
     using C = ColCfg<N, MODE>;
     using X = XPlan<N>;
     constexpr int E = C::E, T = C::T, WC = C::WC;
