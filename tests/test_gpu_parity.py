@@ -743,3 +743,69 @@ def test_single_series_single_pixel_spectrum(torch, B, oracle):
     top = np.argsort(got[0, :, 0])[-2:]
     assert sorted(top.tolist()) == sorted([T // 2 + 5, T // 2 - 9])
     tc.close()
+
+
+def test_guard_bands_around_every_buffer_stay_untouched(torch, B):
+    """Bounds check of our own (compute-sanitizer is closed on this pool): every device buffer the path writes -- the
+    workspace, transmissions, probes, waves, the time-ordered buffer, I(q,E) -- sits between two 1 MiB guard bands filled
+    with a byte pattern; after the whole path (8 frames so that the 2^k spectrum kernel runs, then 5 for the generic DFT)
+    every guard byte is unchanged, and the results equal those of a run on plain allocations bit for bit."""
+    G = 1 << 20
+    wl = W.make_workload(1, nframes=8)
+    seg = wl.segments[0]
+    P, S, n = wl.nprobes, seg.nslices, wl.nx
+    roi = B.make_roi(wl.nx, wl.ny, wl.lx, wl.ly, wl.lam, wl.roi_mode, [p * 1e-3 for p in wl.roi_params_mrad])
+    Q = int(roi.size)
+    sizes = dict(natoms=seg.pos0.shape[0], nframes=8, nslices=S, nsegments=1, nwaves=8 * P, nprobes=P, host_staging=1)
+    guarded = []
+
+    def guard(nbytes):
+        nb = (nbytes + 255) // 256 * 256
+        t = torch.full((nb + 2 * G,), 0xA5, dtype=torch.uint8, device="cuda")
+        assert t.data_ptr() % 256 == 0
+        guarded.append((t, nb))
+        return t[G:G + nb]
+
+    def cplx(shape, guarded_alloc):
+        numel = int(np.prod(shape))
+        if guarded_alloc:
+            return guard(numel * 8)[:numel * 8].view(torch.complex64).view(shape)
+        return torch.empty(shape, dtype=torch.complex64, device="cuda")
+
+    results = []
+    for use_guards in (True, False):
+        tc = B.Tacaw(wl.nx, wl.ny, wl.lx, wl.ly, wl.lam, wl.sigma, wl.bandlimit)
+        nws = tc.workspace_bytes(**sizes)
+        ws = guard(nws)[:nws] if use_guards else torch.empty(nws, dtype=torch.uint8, device="cuda")
+        tc.set_workspace(ws, **sizes)
+        trans = cplx((8, S, n, n), use_guards)
+        probes = cplx((P, n, n), use_guards)
+        waves = cplx((8 * P, n, n), use_guards)
+        buf = cplx((P, 8, Q), use_guards)
+        buf.zero_()
+        I = (guard(P * 8 * Q * 4)[:P * 8 * Q * 4].view(torch.float32) if use_guards
+             else torch.empty(P * 8 * Q, dtype=torch.float32, device="cuda")).view(P, 8, Q)
+        pos = dev(torch, seg.frames(0, 8, wl.dt_fs))
+        tc.build_slices_host(seg.frames(0, 8, wl.dt_fs), seg.species, wl.a, wl.b, wl.dz, S, 0.0, trans, want_clamped=False)
+        t2 = torch.empty_like(trans)
+        tc.build_slices(pos, dev(torch, seg.species), wl.a, wl.b, wl.dz, S, 0.0, out=t2)
+        assert torch.equal(t2, trans)
+        tc.make_probes(wl.probes_xy, wl.alpha_mrad * 1e-3, out=probes)
+        roi_d = dev(torch, roi)
+        inv = tc.make_roi_inverse(roi_d)
+        wf = np.repeat(np.arange(8, dtype=np.int32), P)
+        wp = np.tile(np.arange(P, dtype=np.int32), 8)
+        tr = [[trans[f]] for f in range(8)]
+        tc.propagate_accumulate(waves, wp, wf, wf, tr, wl.dz, inv, Q, buf, probes=probes)
+        tc.propagate(waves, wf, tr, wl.dz, 1, probes=probes, wave_probe=wp)          # unfused pair into the same buffer
+        tc.accumulate(waves, wp, wf, roi_d, buf)
+        Iout, E = tc.spectrum(buf, wl.dt_fs, 1, wl.temperature_K, out=I)
+        I5, _ = tc.spectrum(buf[:, :5].contiguous(), wl.dt_fs, 1, wl.temperature_K)
+        torch.cuda.synchronize()
+        tc.device_status()
+        results.append((trans.clone(), buf.clone(), Iout.clone(), I5.clone()))
+        tc.close()
+    for t, nb in guarded:
+        assert bool((t[:G] == 0xA5).all()) and bool((t[G + nb:] == 0xA5).all())
+    for a, b in zip(*results):
+        assert torch.equal(a, b)
