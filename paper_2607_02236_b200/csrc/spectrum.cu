@@ -103,7 +103,9 @@ struct SpecCfg2 {
     static constexpr int WQ = (N == 512) ? 16 : 8;
     static constexpr int THREADS = T * WQ;
     static constexpr int XE = exch2_elems(N, WQ);
-    static constexpr size_t smem() { return sizeof(float2) * ((size_t)P::TW_ELEMS + XE); }
+    // twiddles | exchange / staging tile | window [N] | Bose factors of the kept bins [<= N]
+    static constexpr size_t smem() { return sizeof(float2) * ((size_t)P::TW_ELEMS + XE) + sizeof(float) * 2 * N; }
+    static_assert(P::TW_ELEMS % 2 == 0 && XE % 2 == 0, "16-byte alignment of the staging tile and of the float tables");
 };
 
 // Persistent: a CTA walks (tile, chunk) work items with stride gridDim.x.  The [T][WQ] tile of the NEXT item is requested
@@ -127,14 +129,37 @@ __global__ void __launch_bounds__(SpecCfg2<N>::THREADS, (SpecCfg2<N>::THREADS >=
     const int c = lt % WQ, tid = lt / WQ;
     float2* tw = smem;
     float2* ex = smem + P::TW_ELEMS;
+    float* sw = reinterpret_cast<float*>(ex + C::XE);             // window and Bose tables: read by every item of this CTA
+    float* sb = sw + N;
     fft2_load_twiddles<N>(tw, table, lt, C::THREADS);
+    for (int i = lt; i < N; i += C::THREADS) {
+        sw[i] = window[i];
+        sb[i] = i < nE ? bose[i] : 0.f;
+    }
+    // even Q (and even strides): a row segment of the tile is 16-byte aligned, so two series go per cp.async
+    const bool vec2 = ((nroi | (long long)probe_stride | (long long)frame_stride | (long long)chunk_stride) & 1) == 0 &&
+                      (reinterpret_cast<uintptr_t>(buf) & 15) == 0;
     const long long ntq = (nroi + WQ - 1) / WQ;
     const long long ntiles = ntq * nprobes;                    // tile = (probe, q tile); a CTA takes tiles blockIdx.x + k gridDim.x
     auto issue = [&](long long tile, int ch) {                 // and runs all chunks of a tile before the next tile
         const int p = (int)(tile / ntq);
         const long long r = (tile - (long long)p * ntq) * WQ + c;
         const float2* src = buf + (size_t)p * probe_stride + (size_t)ch * chunk_stride + r;
-        if (r < nroi) {
+        if (vec2) {
+            const int c2 = 2 * (lt % (WQ / 2)), rb = lt / (WQ / 2);         // series pair, first of this thread's E/2 rows
+            const long long r2 = r - c + c2;
+            const float2* src2 = src - c + c2;
+            if (r2 < nroi) {
+#pragma unroll
+                for (int j = 0; j < E / 2; ++j) cp_async16(ex + (rb + 2 * T * j) * WQ + c2, src2 + (size_t)(rb + 2 * T * j) * frame_stride);
+            } else {
+#pragma unroll
+                for (int j = 0; j < E / 2; ++j) {
+                    ex[(rb + 2 * T * j) * WQ + c2] = make_float2(0.f, 0.f);
+                    ex[(rb + 2 * T * j) * WQ + c2 + 1] = make_float2(0.f, 0.f);
+                }
+            }
+        } else if (r < nroi) {
 #pragma unroll
             for (int m = 0; m < E; ++m) cp_async8(ex + (tid + T * m) * WQ + c, src + (size_t)(tid + T * m) * frame_stride);
         } else {
@@ -161,7 +186,7 @@ __global__ void __launch_bounds__(SpecCfg2<N>::THREADS, (SpecCfg2<N>::THREADS >=
 #pragma unroll
         for (int m = 0; m < E; ++m) {
             const float2 v = ex[(tid + T * m) * WQ + c];
-            const float wm = __ldg(window + tid + T * m);       // 4 N bytes, L1-resident
+            const float wm = sw[tid + T * m];
             x[m] = make_float2(v.x * wm, v.y * wm);
         }
         __syncthreads();                           // tile consumed: the exchange may overwrite it
@@ -190,7 +215,7 @@ __global__ void __launch_bounds__(SpecCfg2<N>::THREADS, (SpecCfg2<N>::THREADS >=
                 for (int m = 0; m < E; ++m) {
                     const int kbin = tid + T * m;
                     const int e = ((kbin + N / 2) & (N - 1)) - e_lo;      // position on the ascending energy axis
-                    if (e >= 0 && e < nE) dst[(size_t)e * nroi] = bose[e] * (WELCH ? acc[m] : x[m].x * x[m].x + x[m].y * x[m].y);
+                    if (e >= 0 && e < nE) dst[(size_t)e * nroi] = sb[e] * (WELCH ? acc[m] : x[m].x * x[m].x + x[m].y * x[m].y);
                 }
             }
         }
