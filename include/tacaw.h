@@ -11,7 +11,9 @@
  *   - Arrays are row-major [iy][ix], x fastest.  complex64 = interleaved (re, im) float.
  *   - Frequency index h = ix for ix < nx/2, else ix - nx (same for k, iy).  q = (h/lx, k/ly) in
  *     1/Angstrom (no 2 pi).  Forward transform uses exp(-2 pi i ...); inverse carries 1/(nx ny).
- *   - nx, ny: powers of two in [16, 2048] (they may differ).
+ *   - nx, ny in [16, 2048] (they may differ): powers of two run on the register FFTs of the tuned kernels; any other EVEN
+ *     size whose prime factors are 2, 3, 5, 7 only (the paper's 1680 = 2^4 3 5 7) runs on a plain mixed-radix
+ *     path (same results and tolerances, several times slower).  Anything else: TACAW_E_UNSUPPORTED.
  *   - Every "d_" pointer is DEVICE memory owned by the caller; the library never frees or
  *     reallocates it.  The library owns only the context (twiddle / propagator tables, a pinned host
  *     arena for index uploads, streams and events) -- all created in tacaw_create.  Scratch for the

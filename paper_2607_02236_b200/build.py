@@ -9,7 +9,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtacaw.so")
-SOURCES = ["api.cu", "propagate.cu", "potential.cu", "potential_tc.cu", "spectrum.cu"]
+SOURCES = ["api.cu", "propagate.cu", "potential.cu", "potential_tc.cu", "spectrum.cu", "generic.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr", "-Xptxas", "-v"]
 

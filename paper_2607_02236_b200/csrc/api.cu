@@ -42,7 +42,7 @@ static void region_sizes(const tacaw_ctx* ctx, const tacaw_sizes& z, size_t (&by
     bytes[tacaw_ctx::R_STAGE] = z.host_staging ? up(sizeof(double) * 3 * natoms * nframes + sizeof(int32_t) * natoms + 64) : 0;
     bytes[tacaw_ctx::R_PROBE] = up(sizeof(int) * (size_t)ctx->grid.nx + sizeof(uint32_t) * 2 * nprobes + 64);
     // propagate: wave_frame | wave_probe | tuples (<= (nwaves + 64) * rpt) | transmission pointers
-    const size_t rpt = (size_t)row_tuple_size(ctx->grid.nx);
+    const size_t rpt = ctx->generic_path ? 1 : (size_t)row_tuple_size(ctx->grid.nx);
     bytes[tacaw_ctx::R_PROP] = up(sizeof(int) * (3 * nwaves + (nwaves + 64) * rpt) + 16 + sizeof(void*) * nframes * nseg + 64);
     bytes[tacaw_ctx::R_ACC] = up(sizeof(int) * 2 * nwaves + 64);
     bytes[tacaw_ctx::R_SPEC] = up(SPEC_TABLE_BYTES);
@@ -84,10 +84,16 @@ static bool mask_in_band(int h, int k, const tacaw_grid& g) {
     return qx * qx + qy * qy <= (4.0 / 9.0) * qn * qn;
 }
 
-static bool supported_n(int n) { return n >= 16 && n <= 2048 && (n & (n - 1)) == 0; }
+// powers of two in [16, 2048] run on the register FFTs; other even sizes with prime factors 2, 3, 5, 7 on generic.cu
+static bool supported_n(int n) { return (n >= 16 && n <= 2048 && (n & (n - 1)) == 0) || generic_grid_supported(n); }
 
 // twiddle table of the slice-step transforms of length n (layout: fft2.cuh)
-static void make_roots(int n, std::vector<float2>& out) {
+static void make_roots(int n, bool generic, std::vector<float2>& out) {
+    if (generic) {                       // generic.cu: the n-th roots of unity
+        out.resize(n);
+        generic_host_table(n, out.data());
+        return;
+    }
     out.resize(slice_step_table_elems(n));
     slice_step_host_table(n, out.data());
 }
@@ -181,8 +187,10 @@ int tacaw_create(tacaw_ctx** out, const tacaw_grid* grid, const tacaw_beam* beam
         if (km > ctx->kmaxmax) ctx->kmaxmax = km;
     }
     std::vector<float2> rx, ry;
-    make_roots(nx, rx);
-    make_roots(ny, ry);
+    const auto pow2 = [](int n) { return (n & (n - 1)) == 0; };
+    ctx->generic_path = !pow2(nx) || !pow2(ny);       // one dimension off the powers of two puts both passes on generic.cu
+    make_roots(nx, ctx->generic_path, rx);
+    make_roots(ny, ctx->generic_path, ry);
     bool ok = cudaMalloc(&ctx->d_roots_x, sizeof(float2) * rx.size()) == cudaSuccess &&
               cudaMalloc(&ctx->d_roots_y, sizeof(float2) * ry.size()) == cudaSuccess &&
               cudaMalloc(&ctx->d_kmax, sizeof(int) * nx) == cudaSuccess &&
@@ -469,7 +477,7 @@ static int propagate_impl(tacaw_ctx* ctx, void* d_waves, const void* d_probes, i
     const tacaw_grid& g = ctx->grid;
     const size_t npix = (size_t)g.nx * g.ny;
     // metadata: [wave_frame nwaves][wave_probe nwaves][wave_slot nwaves][tuples <= nwaves*rpt][trans ptrs nframes*nseg]
-    const int rpt = row_tuple_size(g.nx);
+    const int rpt = ctx->generic_path ? 1 : row_tuple_size(g.nx);
     size_t nb_i = sizeof(int) * (size_t)nwaves;
     size_t nb_t = sizeof(int) * ((size_t)nwaves + 64) * rpt;
     size_t off_t = 3 * nb_i;

@@ -28,6 +28,8 @@ struct tacaw_ctx {
     int kmaxmax_pot = 0;
     int kmaxmax = 0;              // largest kmax[ix]
 
+    bool generic_path = false;    // nx or ny is not a power of two: both passes run on generic.cu (tables = plain roots of unity)
+
     double dz_cached = -1.0;
     float2* d_px = nullptr;  // [nx] exp(-i pi lambda dz h^2/lx^2) / nx
     float2* d_py = nullptr;  // [ny] exp(-i pi lambda dz k^2/ly^2) / ny
@@ -151,6 +153,11 @@ int row_tuple_size(int nx);        // waves per tuple of the row kernel for this
 int slice_step_table_elems(int n); // twiddle table of the slice-step transforms of length n (fft2.cuh XPlan layout) ...
 void slice_step_host_table(int n, float2* tab);   // ... built on the host in fp64
 int launch_col(tacaw_ctx* ctx, int mode, const ColArgs& a, int ny, cudaStream_t st);
+// grids that are not powers of two (generic.cu): even n <= 2048 with prime factors 2, 3, 5, 7 (the paper's 1680)
+bool generic_grid_supported(int n);
+int launch_row_generic(tacaw_ctx* ctx, int mode, const RowArgs& a, cudaStream_t st);
+int launch_col_generic(tacaw_ctx* ctx, int mode, const ColArgs& a, int ny, cudaStream_t st);
+void generic_host_table(int n, float2* tab);      // n roots of unity exp(-2 pi i m / n)
 
 // d_nclamped (out): device address of this call's clamp counter inside the build region
 int launch_potential(tacaw_ctx* ctx, const double* d_pos, const int32_t* d_species, int natoms, int nframes, int nspecies,

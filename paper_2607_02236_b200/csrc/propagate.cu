@@ -420,6 +420,7 @@ void slice_step_host_table(int n, float2* tab) { xplan_host_table(n, tab); }
 
 int launch_row(tacaw_ctx* ctx, int mode, const RowArgs& a, cudaStream_t st) {
     if (a.nwaves <= 0) return TACAW_OK;
+    if (ctx->generic_path) return launch_row_generic(ctx, mode, a, st);      // a grid edge that is not a power of two
     switch (ctx->grid.nx) {
         case 16: return launch_row_mode<16>(ctx, mode, a, st);
         case 32: return launch_row_mode<32>(ctx, mode, a, st);
@@ -430,7 +431,7 @@ int launch_row(tacaw_ctx* ctx, int mode, const RowArgs& a, cudaStream_t st) {
         case 1024: return launch_row_mode<1024>(ctx, mode, a, st);
         case 2048: return launch_row_mode<2048>(ctx, mode, a, st);
     }
-    return fail(ctx, TACAW_E_UNSUPPORTED, "nx must be a power of two in [16, 2048]");
+    return fail(ctx, TACAW_E_UNSUPPORTED, "nx must be a power of two in [16, 2048] on this path");
 }
 
 // ------------------------------------------------------------------------------------------
@@ -734,6 +735,7 @@ static int launch_col_mode(tacaw_ctx* ctx, int mode, const ColArgs& a, cudaStrea
 
 int launch_col(tacaw_ctx* ctx, int mode, const ColArgs& a, int ny, cudaStream_t st) {
     if (a.nwaves <= 0) return TACAW_OK;
+    if (ctx->generic_path) return launch_col_generic(ctx, mode, a, ny, st);
     switch (ny) {
         case 16: return launch_col_mode<16>(ctx, mode, a, st);
         case 32: return launch_col_mode<32>(ctx, mode, a, st);
@@ -744,7 +746,7 @@ int launch_col(tacaw_ctx* ctx, int mode, const ColArgs& a, int ny, cudaStream_t 
         case 1024: return launch_col_mode<1024>(ctx, mode, a, st);
         case 2048: return launch_col_mode<2048>(ctx, mode, a, st);
     }
-    return fail(ctx, TACAW_E_UNSUPPORTED, "ny must be a power of two in [16, 2048]");
+    return fail(ctx, TACAW_E_UNSUPPORTED, "ny must be a power of two in [16, 2048] on this path");
 }
 
 }  // namespace tacaw

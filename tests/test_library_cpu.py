@@ -43,7 +43,8 @@ def test_create_fails_loudly_without_gpu(lib):
 def test_create_rejects_unsupported_grids(lib):
     ctx = C.c_void_p()
     b = binding._Beam(0.037, 9e-4, 1)
-    for nx, ny in ((48, 64), (8, 64), (64, 4096), (0, 0)):
+    # supported: powers of two in [16, 2048] and other even sizes in that range with prime factors 2, 3, 5, 7 only
+    for nx, ny in ((46, 64), (63, 64), (8, 64), (64, 4096), (64, 2046), (0, 0)):
         g = binding._Grid(nx, ny, 10.0, 10.0)
         assert lib.tacaw_create(C.byref(ctx), C.byref(g), C.byref(b), 0) == -2  # TACAW_E_UNSUPPORTED
 
