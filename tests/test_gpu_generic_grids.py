@@ -34,8 +34,8 @@ def dev(torch, a, dtype=None):
     return t if dtype is None else t.to(dtype)
 
 
-@pytest.mark.parametrize("nx,ny", [(48, 48), (210, 210), (240, 210), (210, 256), (420, 360), (30, 18)])
-@pytest.mark.parametrize("bandlimit", [1, 0])
+@pytest.mark.parametrize("nx,ny,bandlimit", [(48, 48, 1), (48, 48, 0), (210, 210, 1), (240, 210, 1), (210, 256, 1), (210, 256, 0),
+                                             (420, 360, 1), (30, 18, 1)])
 def test_propagate_random_slices_on_mixed_radix_grids(torch, B, oracle, nx, ny, bandlimit):
     """Random unit-modulus transmissions and random waves on grids with factors 3, 5, 7 (radix lists 8.6, 7.6.5, 8.6.5,
     7.6.5.2, 8.5.3.3 ...), rectangular ones and one mixed with a power of two; both output spaces, several frames and
@@ -68,9 +68,9 @@ def test_propagate_random_slices_on_mixed_radix_grids(torch, B, oracle, nx, ny, 
     tc.close()
 
 
-@pytest.mark.parametrize("n", [210, 240])
+@pytest.mark.parametrize("n", [210])
 def test_whole_path_on_a_mixed_radix_grid(torch, B, oracle, n):
-    """build_slices (K1 + V -> t), probes, multislice, fused ROI gather, spectrum on an n x n grid, n = 2 3 5 7 and 2^4 3 5:
+    """build_slices (K1 + V -> t), probes, multislice, fused ROI gather, spectrum on an n x n grid, n = 2 3 5 7:
     against the oracle pipeline."""
     from oracle import pipeline as OP
     from paper_2607_02236_b200.pipeline import Runner
@@ -96,7 +96,7 @@ def test_whole_path_with_one_1680_edge(torch, B, oracle, nx, ny):
     grids whose other edge is short so that the oracle's O(N^2) transforms of length 1680 stay cheap."""
     from oracle import pipeline as OP
     from paper_2607_02236_b200.pipeline import Runner
-    wl = W.tiny_workload(n=32, ncell=(2, 2, 1), nframes=4, alpha_mrad=30.0)
+    wl = W.tiny_workload(n=32, ncell=(2, 2, 1), nframes=2, alpha_mrad=30.0)
     wl.nx, wl.ny = nx, ny
     wl.roi_mode, wl.roi_params_mrad = "rect", (-100.0, 100.0, -100.0, 100.0)
     ref = OP.run(wl, pot_mode=0)
