@@ -13,7 +13,8 @@ Consecutive steps take consecutive frame blocks, so the default 4 timed steps co
            region through tacaw_build_slices_host, the spectrum I(q,E) copied back D2H).
 `roofline`: the fused slice-step kernel pair (k_row + k_col), algorithmic bytes B_step = 16 N^2 + 8 N^2/R per wave and slice
             over the CUDA-event time of the tacaw_propagate_accumulate calls inside the timed region.
-`roofline_by_grid`: the same fraction measured in the same run on short samples of configs[2] (512^2) and configs[3] (1024^2).
+`roofline_by_grid`: the same fraction measured in the same run on short samples of configs[2] (512^2) and configs[3] (1024^2),
+           and on the paper's own 1680^2 grid (mixed-radix path).
 `comparison`: cuFFT plan-many and torch.fft.fft2 slice loops on the same grid (library baselines, not the product).
 `cpu_baseline`: the fp64 oracle, as it stands, on a bounded sample of the same workload.
 `--impl reference` times the oracle alone (this tier's reference arm).
@@ -283,6 +284,34 @@ def propagate_only(torch, cfg, nframes, reps, peak):
             "ms": ms}
 
 
+def generic_grid_sample(torch, n, nwaves, nslices, reps, peak):
+    """roofline_by_grid: the paper's own grid edge, 1680 = 2^4 3 5 7, which runs on the plain mixed-radix kernels
+    of csrc/generic.cu: `nwaves` random unit-norm waves of one frame through `nslices` random unit-modulus transmissions."""
+    from paper_2607_02236_b200 import binding as B
+    tc = B.Tacaw(n, n, 93.0, 93.0, 0.0487, 9.2e-4, 1)
+    g = torch.Generator(device="cuda").manual_seed(1680)
+    t = torch.polar(torch.ones((nslices, n, n), device="cuda"), torch.randn((nslices, n, n), device="cuda", generator=g)).to(torch.complex64)
+    w = torch.randn((nwaves, n, n), dtype=torch.complex64, device="cuda", generator=g)
+    w /= torch.linalg.vector_norm(w, dim=(1, 2), keepdim=True)
+    wf = np.zeros(nwaves, np.int32)
+    tc.propagate(w, wf, [[t]], 1.5, 1)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        tc.propagate(w, wf, [[t]], 1.5, 1)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / reps
+    rate = nwaves * nslices / (ms * 1e-3)
+    b = 16 * n * n + 8 * n * n / nwaves
+    tc.close()
+    return {"workload": f"{n}x{n} (the paper's grid; mixed-radix path of csrc/generic.cu, not tuned), {nwaves} waves x {nslices} random slices "
+                        "(tacaw_propagate only)",
+            "propagate_slice_steps_per_s": rate, "bytes_per_slice_step": b, "achieved_GBps": rate * b / 1e9, "frac": rate * b / 1e9 / peak,
+            "ms": ms}
+
+
 def measured_traffic(wl_name):
     """dram__bytes_read.sum + dram__bytes_write.sum of the slice-step pair per wave and slice, from the committed ncu --set full
     capture -- used only if that capture was taken at exactly the kernel sources this run was built from."""
@@ -493,6 +522,11 @@ def main():
             except Exception as ex:  # pragma: no cover
                 by_grid[f"c{cfg}"] = {"error": str(ex)[:200]}
             torch.cuda.empty_cache()
+        try:
+            by_grid["paper_1680"] = generic_grid_sample(torch, 1680, 16, 8, 3, peak)
+        except Exception as ex:  # pragma: no cover
+            by_grid["paper_1680"] = {"error": str(ex)[:200]}
+        torch.cuda.empty_cache()
         nw_c = {2048: 16, 1024: 64}.get(wl.nx, 128)
         comparison = comparison_arms(torch, dev, wl.nx, min(nw_c, max(R, 1)) if wl.nx >= 1024 else nw_c, 8, b_step, peak)
         comparison["note"] = ("library baselines on this grid, same byte model; each slice step = 2 batched 2D FFT calls + 2 elementwise passes "

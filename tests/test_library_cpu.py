@@ -49,6 +49,19 @@ def test_create_rejects_unsupported_grids(lib):
         assert lib.tacaw_create(C.byref(ctx), C.byref(g), C.byref(b), 0) == -2  # TACAW_E_UNSUPPORTED
 
 
+def test_create_accepts_the_papers_1680_grid_and_other_2357_sizes(lib):
+    """Even sizes in [16, 2048] whose prime factors are 2, 3, 5, 7 pass the size check (1680 = 2^4 3 5 7): without
+    a GPU the call then fails with TACAW_E_CUDA (-4), never with TACAW_E_UNSUPPORTED (-2)."""
+    b = binding._Beam(0.037, 9e-4, 1)
+    for nx, ny in ((1680, 1680), (210, 256), (48, 16), (2048, 1680), (1260, 420)):
+        ctx = C.c_void_p()
+        g = binding._Grid(nx, ny, 10.0, 10.0)
+        rc = lib.tacaw_create(C.byref(ctx), C.byref(g), C.byref(b), 0)
+        assert rc in (0, -4), (nx, ny, rc)
+        if rc == 0:
+            lib.tacaw_destroy(ctx)
+
+
 @pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
 def test_roi_map_bit_exact_all_configs(lib, oracle, cfg):
     wl = W.make_workload(cfg, nframes=1, nprobes=1, ncz=1 if cfg >= 3 else None)
